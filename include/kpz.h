@@ -1,0 +1,147 @@
+/* kpz.h -- C ABI of the B200-native octahedron-KPZ hot path (libkpz_b200.so).
+ *
+ * Method: Kelling & Odor, "Extremely large scale simulation of a Kardar-Parisi-Zhang model using graphics
+ * cards", arXiv:1110.6745 (PAPER.md; "P:n" = PAPER.md line n).  The library advances a periodic L x L lattice of
+ * slopes sigma_x, sigma_y in {+-1} (2 bits per site) by stochastic generalized-Kawasaki updates (eq. 2,
+ * P:26-30) under the deterministic domain-decomposed random-sequential schedule of DESIGN.md section "Schedule"
+ * (random origin per MCS in multiples of 4 sites; 4 tile colours in random order; T*T sequential
+ * attempts per tile; every random number from Philox4x32-10 keyed by (seed; call, tile, MCS, replica)), and
+ * reduces heights (eq. 3) to sum h, sum h^2 and the squared width W^2 (eq. 4).
+ *
+ * Conventions
+ *   - All functions return an int32_t status: KPZ_OK (0) or a negative KPZ_E* code.  Nothing throws or aborts.
+ *     kpz_last_error(ctx) returns a NUL-terminated message owned by the handle (valid until the next call on it).
+ *   - "host" / "device" is stated for every pointer.  The caller owns every buffer it passes; the library owns
+ *     only the opaque handle (freed by kpz_destroy) and small temporaries it allocates inside diagnostic calls.
+ *   - Device buffers are allocated by the caller (PyTorch in the Python binding) and bound with kpz_bind; they
+ *     must outlive the handle or be re-bound.  All work is enqueued on the bound CUDA stream.
+ *   - A handle is not thread-safe; distinct handles are independent.
+ *   - Coordinates are 0-based, x fastest: host slope arrays are row-major [y*L + x], values +1 / -1, with
+ *     sigma_x(x,y) = h(x,y) - h(x-1,y) and sigma_y(x,y) = h(x,y) - h(x,y-1) (indices mod L, R3).
+ *   - There is no CPU fallback: without a CUDA device every call that needs one returns KPZ_ECUDA.
+ *
+ * Device layout of the lattice buffer, per replica r at byte offset
+ * r * L*L/4:  plane X = sigma_x as L bit-lines, one per COLUMN x (32-bit words, bit (y & 31) of word
+ * x*(L/32) + (y >> 5)), followed by plane Y = sigma_y as L bit-lines, one per ROW y (bit (x & 31) of word
+ * y*(L/32) + (x >> 5)).  Bit 1 <=> sigma = +1.
+ */
+#ifndef KPZ_B200_H
+#define KPZ_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define KPZ_OK 0
+#define KPZ_EINVAL (-1)    /* bad argument (size, tile, probability, NULL pointer, replica out of range) */
+#define KPZ_ENOMEM (-2)    /* a bound buffer is too small / temporary allocation failed */
+#define KPZ_ECUDA (-3)     /* CUDA runtime error or no device; message in kpz_last_error */
+#define KPZ_EOVERFLOW (-4) /* a requested int64 output does not fit (kpz_measure) */
+#define KPZ_ESTATE (-5)    /* call order (not bound) or an invalid lattice state (kpz_set_slopes) */
+
+typedef struct kpz_ctx kpz_ctx;
+
+/* Sizes of the two device buffers kpz_bind expects, in bytes (host out-pointers).
+ * lattice = n_replicas * L*L/4 (2 bits per site).  scratch holds per-replica counters and the partial
+ * sums of the measurement kernels.  Same argument rules as kpz_create_batch; KPZ_EINVAL otherwise. */
+int32_t kpz_workspace_bytes(uint32_t L, uint32_t tile, uint32_t n_replicas, size_t* lattice_bytes,
+                            size_t* scratch_bytes);
+
+/* Creates a handle for one lattice (north star signature kpz_create(L, p, q, tile, seed)).
+ *   L    : linear size; a multiple of 2*tile and of 32.
+ *   p, q : deposition / removal probabilities of eq. 2, each in [0,1]; accept iff a 32-bit Philox word
+ *          is < floor(prob * 2^32) (always for prob = 1).
+ *   tile : tile edge T, one of 4, 8, 16, 32, 64 (a power of two >= 4, multiples-of-4 offsets).
+ *   seed : 64-bit Philox key.
+ * *out receives the handle (host pointer).  Errors: KPZ_EINVAL, KPZ_ECUDA (no device). */
+int32_t kpz_create(kpz_ctx** out, uint32_t L, double p, double q, uint32_t tile, uint64_t seed);
+
+/* As kpz_create, for n_replicas >= 1 independent lattices ("independent runs") advanced together.
+ * Replica r uses Philox counter word c3 = r; kpz_create == kpz_create_batch(..., 1). */
+int32_t kpz_create_batch(kpz_ctx** out, uint32_t L, double p, double q, uint32_t tile, uint64_t seed,
+                         uint32_t n_replicas);
+
+/* Binds caller-owned DEVICE buffers (sizes from kpz_workspace_bytes; 16-byte aligned) and a CUDA stream
+ * (cudaStream_t passed as void*, NULL = default stream).  Zeroes the scratch counters (asynchronously).
+ * The lattice content is left as is.  lattice_bytes / scratch_bytes are the sizes the caller allocated;
+ * KPZ_ENOMEM if too small. */
+int32_t kpz_bind(kpz_ctx* ctx, void* d_lattice, size_t lattice_bytes, void* d_scratch, size_t scratch_bytes,
+                 void* cuda_stream);
+
+/* Flat zig-zag start of P:88: h(x,y) = (x+y) mod 2, i.e. sigma_x = sigma_y = +1 if (x+y) odd else -1;
+ * W^2 = 1/4.  Resets h(0,0) = 0, the MCS clock and all counters of every replica.  Asynchronous. */
+int32_t kpz_init_flat(kpz_ctx* ctx);
+
+/* Advances every replica by `mcs` Monte Carlo steps (each exactly L*L attempts, 4 kernel launches).
+ * Asynchronous on the bound stream.  kpz_run(a); kpz_run(b) == kpz_run(a+b).  KPZ_EINVAL if the MCS clock
+ * would pass 2^32 - 1 (it is a 32-bit Philox counter word). */
+int32_t kpz_run(kpz_ctx* ctx, uint64_t mcs);
+
+/* Height reconstruction (eq. 3) and width (eq. 4).  HOST out-arrays of length n_replicas (any may be NULL).
+ * sum_h, sum_h2: exact sums over all sites of h and h^2 with absolute heights anchored by h(0,0) (tracked:
+ * 0 at kpz_init_flat, +-2 per accepted flip at site (0,0)).  W2 = (N*sum_h2 - sum_h^2)/N^2, N = L*L, from
+ * 128-bit integers: one conversion to double, one division by (double)N^2.  Synchronises the stream.
+ * Does not modify the lattice.  KPZ_EOVERFLOW if a requested sum does not fit int64 (W2 is still written). */
+int32_t kpz_measure(kpz_ctx* ctx, int64_t* sum_h, int64_t* sum_h2, double* W2);
+
+/* Frees the handle (not the bound buffers).  NULL is a no-op. */
+int32_t kpz_destroy(kpz_ctx* ctx);
+
+/* Waits for all work enqueued on the bound stream. */
+int32_t kpz_synchronize(kpz_ctx* ctx);
+
+const char* kpz_last_error(const kpz_ctx* ctx);
+
+/* ---- parity / diagnostic / checkpoint extensions --------------------------------------------------------- */
+
+/* Unpacks replica `replica` into HOST arrays sx, sy (int8, L*L each, row-major [y*L+x], values +-1).
+ * Synchronises.  Allocates 2*L*L bytes of temporary device memory (KPZ_ENOMEM if that fails). */
+int32_t kpz_get_slopes(kpz_ctx* ctx, uint32_t replica, int8_t* sx, int8_t* sy);
+
+/* As kpz_get_slopes for the w x h window with lower-left site (x0, y0), periodic wrap; out arrays [j*w + i]. */
+int32_t kpz_get_window(kpz_ctx* ctx, uint32_t replica, uint32_t x0, uint32_t y0, uint32_t w, uint32_t h,
+                       int8_t* sx, int8_t* sy);
+
+/* Packs HOST arrays (values must be +-1, else KPZ_EINVAL; the state must be curl-free with zero tilt --
+ * sx(x+1,y)+sy(x+1,y+1) = sy(x,y+1)+sx(x+1,y+1), every row sum of sx and column sum of sy zero -- else
+ * KPZ_ESTATE and the replica is left unchanged) into replica `replica`, and sets its h(0,0) to h00.
+ * Does not touch the MCS clock or the flip counters.  Synchronises. */
+int32_t kpz_set_slopes(kpz_ctx* ctx, uint32_t replica, const int8_t* sx, const int8_t* sy, int64_t h00);
+
+/* Order-independent 64-bit hash of replica's state: sum over sites n = y*L+x of
+ * bit_x(n)*mix64(2n) + bit_y(n)*mix64(2n+1) mod 2^64, bit = (sigma+1)/2, mix64 = splitmix64 finaliser
+ * (z += 0x9E3779B97F4A7C15; z = (z^(z>>30))*0xBF58476D1CE4E5B9; z = (z^(z>>27))*0x94D049BB133111EB; z^(z>>31)).
+ * HOST out-pointer.  Synchronises. */
+int32_t kpz_state_hash(kpz_ctx* ctx, uint32_t replica, uint64_t* out);
+
+/* Per-replica counters since kpz_init_flat (HOST out-pointers, any may be NULL): attempted updates
+ * (= mcs * L*L), accepted depositions and removals, tracked height of site (0,0), completed MCS.  Synchronises. */
+int32_t kpz_counters(kpz_ctx* ctx, uint32_t replica, uint64_t* attempts, uint64_t* deposits, uint64_t* removals,
+                     int64_t* h00, uint64_t* mcs);
+
+/* Checkpoint: copies the packed lattice of ALL replicas (device layout above, kpz_workspace_bytes'
+ * lattice_bytes bytes) between the bound device buffer and a HOST buffer (pinned memory makes the copy
+ * asynchronous-capable; the calls synchronise before returning).  kpz_import_packed also takes the state the
+ * lattice does not carry: per-replica h(0,0) (HOST array of n_replicas, NULL = zeros) and the MCS clock. */
+int32_t kpz_export_packed(kpz_ctx* ctx, void* host_dst, size_t bytes);
+int32_t kpz_import_packed(kpz_ctx* ctx, const void* host_src, size_t bytes, const int64_t* h00, uint64_t mcs);
+
+/* End-to-end step with HOST buffers: kpz_import_packed(host_lattice) + kpz_run(mcs) + kpz_measure(...) +
+ * kpz_export_packed(host_lattice), i.e. host->device and device->host copies inside the call (bench.py "e2e"). */
+int32_t kpz_step_host(kpz_ctx* ctx, void* host_lattice, size_t bytes, int64_t* h00_inout, uint64_t mcs_start,
+                      uint64_t mcs, int64_t* sum_h, int64_t* sum_h2, double* W2);
+
+/* Number of kernels this handle has launched since creation (for bench.py "gpu_launches"). */
+int32_t kpz_launch_count(const kpz_ctx* ctx, uint64_t* out);
+
+/* Device Philox4x32-10 self-test: evaluates n (counter,key) inputs on the GPU.  HOST arrays: ctr[4n], key[2n],
+ * out[4n].  Used by the tests to check the in-kernel generator against the published known answers. */
+int32_t kpz_philox_selftest(const uint32_t* ctr, const uint32_t* key, uint32_t* out, uint32_t n);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KPZ_B200_H */

@@ -165,12 +165,12 @@ void run_tile(Oracle* o, uint32_t m, uint32_t ox, uint32_t oy, uint32_t tx, uint
 
 bool tile_touches_window(const Oracle* o, uint32_t ox, uint32_t oy, uint32_t tx, uint32_t ty) {
     if (o->full) return true;
-    // tile covers x in [ox+tx*T, +T) mod L; conservative: test whether any tile column/row lies in the window
-    bool hitx = false, hity = false;
-    for (uint32_t l = 0; l < o->T && !hitx; ++l)
-        if (((ox + tx * o->T + l) % o->L + o->L - o->wx0) % o->L < o->ww) hitx = true;
-    for (uint32_t l = 0; l < o->T && !hity; ++l)
-        if (((oy + ty * o->T + l) % o->L + o->L - o->wy0) % o->L < o->wh) hity = true;
+    // tile covers x in [sx0, sx0+T) mod L, the window covers [wx0, wx0+ww) mod L: two periodic intervals meet
+    // iff the start of one lies inside the other.
+    const uint32_t L = o->L, T = o->T;
+    const uint32_t sx0 = (ox + tx * T) % L, sy0 = (oy + ty * T) % L;
+    const bool hitx = ((sx0 + L - o->wx0) % L < o->ww) || ((o->wx0 + L - sx0) % L < T);
+    const bool hity = ((sy0 + L - o->wy0) % L < o->wh) || ((o->wy0 + L - sy0) % L < T);
     return hitx && hity;
 }
 
@@ -185,7 +185,7 @@ void run_one_mcs(Oracle* o) {
         uint64_t n_dep = 0, n_rem = 0;
         int64_t dh00 = 0;
         const int64_t half = NT / 2;
-        #pragma omp parallel for collapse(2) reduction(+ : n_dep, n_rem, dh00) schedule(static) num_threads(o->nthreads)
+        #pragma omp parallel for collapse(2) reduction(+ : n_dep, n_rem, dh00) schedule(dynamic, 16) num_threads(o->nthreads)
         for (int64_t j = 0; j < half; ++j) {
             for (int64_t k = 0; k < half; ++k) {
                 uint32_t ty = (uint32_t)(2 * j) + cy, tx = (uint32_t)(2 * k) + cx;

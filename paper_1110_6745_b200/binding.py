@@ -1,0 +1,199 @@
+"""ctypes binding of include/kpz.h -- argument marshalling only; every step of the path runs in the CUDA kernels.
+
+Names mirror the C ABI: KPZ.init_flat -> kpz_init_flat, KPZ.run -> kpz_run, KPZ.measure -> kpz_measure, ...
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+import numpy as np
+
+KPZ_OK, KPZ_EINVAL, KPZ_ENOMEM, KPZ_ECUDA, KPZ_EOVERFLOW, KPZ_ESTATE = 0, -1, -2, -3, -4, -5
+_CODES = {KPZ_EINVAL: "KPZ_EINVAL", KPZ_ENOMEM: "KPZ_ENOMEM", KPZ_ECUDA: "KPZ_ECUDA",
+          KPZ_EOVERFLOW: "KPZ_EOVERFLOW", KPZ_ESTATE: "KPZ_ESTATE"}
+
+_LIB_PATH = Path(__file__).resolve().parent / "libkpz_b200.so"
+_lib = None
+
+# every symbol include/kpz.h declares
+exported_symbols = [
+    "kpz_workspace_bytes", "kpz_create", "kpz_create_batch", "kpz_bind", "kpz_init_flat", "kpz_run", "kpz_measure",
+    "kpz_destroy", "kpz_synchronize", "kpz_last_error", "kpz_get_slopes", "kpz_get_window", "kpz_set_slopes",
+    "kpz_state_hash", "kpz_counters", "kpz_export_packed", "kpz_import_packed", "kpz_step_host",
+    "kpz_launch_count", "kpz_philox_selftest",
+]
+
+
+class KpzError(RuntimeError):
+    def __init__(self, code, msg=""):
+        super().__init__("%s (%d)%s" % (_CODES.get(code, "KPZ_E?"), code, ": " + msg if msg else ""))
+        self.code = code
+
+
+def load_library() -> ctypes.CDLL:
+    """Loads the compiled extension; fails loudly if it is missing (no fallback of any kind)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not _LIB_PATH.exists():
+        raise ImportError("%s is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                          "(nvcc, sm_100a) first -- there is no CPU fallback" % _LIB_PATH)
+    L = ctypes.CDLL(str(_LIB_PATH))
+    vp, u32, u64, i64, dbl, i32, sz = (ctypes.c_void_p, ctypes.c_uint32, ctypes.c_uint64, ctypes.c_int64,
+                                       ctypes.c_double, ctypes.c_int32, ctypes.c_size_t)
+    sig = {
+        "kpz_workspace_bytes": [u32, u32, u32, vp, vp],
+        "kpz_create": [vp, u32, dbl, dbl, u32, u64],
+        "kpz_create_batch": [vp, u32, dbl, dbl, u32, u64, u32],
+        "kpz_bind": [vp, vp, sz, vp, sz, vp],
+        "kpz_init_flat": [vp],
+        "kpz_run": [vp, u64],
+        "kpz_measure": [vp, vp, vp, vp],
+        "kpz_destroy": [vp],
+        "kpz_synchronize": [vp],
+        "kpz_get_slopes": [vp, u32, vp, vp],
+        "kpz_get_window": [vp, u32, u32, u32, u32, u32, vp, vp],
+        "kpz_set_slopes": [vp, u32, vp, vp, i64],
+        "kpz_state_hash": [vp, u32, vp],
+        "kpz_counters": [vp, u32, vp, vp, vp, vp, vp],
+        "kpz_export_packed": [vp, vp, sz],
+        "kpz_import_packed": [vp, vp, sz, vp, u64],
+        "kpz_step_host": [vp, vp, sz, vp, u64, u64, vp, vp, vp],
+        "kpz_launch_count": [vp, vp],
+        "kpz_philox_selftest": [vp, vp, vp, u32],
+    }
+    for name, args in sig.items():
+        fn = getattr(L, name)
+        fn.argtypes = args
+        fn.restype = i32
+    L.kpz_last_error.argtypes = [vp]
+    L.kpz_last_error.restype = ctypes.c_char_p
+    _lib = L
+    return L
+
+
+def workspace_bytes(L, tile, n_replicas=1):
+    a, b = ctypes.c_size_t(), ctypes.c_size_t()
+    rc = load_library().kpz_workspace_bytes(L, tile, n_replicas, ctypes.addressof(a), ctypes.addressof(b))
+    if rc != KPZ_OK:
+        raise KpzError(rc)
+    return a.value, b.value
+
+
+def philox_selftest(ctr, key):
+    ctr = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
+    key = np.ascontiguousarray(key, dtype=np.uint32).reshape(-1, 2)
+    out = np.zeros_like(ctr)
+    rc = load_library().kpz_philox_selftest(ctr.ctypes.data, key.ctypes.data, out.ctypes.data, len(ctr))
+    if rc != KPZ_OK:
+        raise KpzError(rc)
+    return out
+
+
+class KPZ:
+    """One handle = n_replicas lattices of size L x L (kpz_create_batch + kpz_bind with torch-allocated buffers)."""
+
+    def __init__(self, L, p, q, tile, seed, n_replicas=1, device="cuda:0", stream=None):
+        import torch
+        self._torch = torch
+        self._lib = load_library()
+        self._h = ctypes.c_void_p()
+        self.L, self.p, self.q, self.tile, self.seed, self.n_replicas = L, p, q, tile, seed, n_replicas
+        rc = self._lib.kpz_create_batch(ctypes.addressof(self._h), L, float(p), float(q), tile, seed, n_replicas)
+        if rc != KPZ_OK:
+            self._h = ctypes.c_void_p()
+            raise KpzError(rc, "kpz_create_batch")
+        self.lattice_bytes, self.scratch_bytes = workspace_bytes(L, tile, n_replicas)
+        self.device = torch.device(device)
+        with torch.cuda.device(self.device):
+            self.lattice = torch.empty(self.lattice_bytes, dtype=torch.uint8, device=self.device)
+            self.scratch = torch.empty(self.scratch_bytes, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            self._check(self._lib.kpz_bind(self._h, self.lattice.data_ptr(), self.lattice_bytes,
+                                           self.scratch.data_ptr(), self.scratch_bytes, self.stream.cuda_stream))
+
+    def _check(self, rc, allow=()):
+        if rc != KPZ_OK and rc not in allow:
+            msg = self._lib.kpz_last_error(self._h)
+            raise KpzError(rc, msg.decode() if msg else "")
+        return rc
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            self._lib.kpz_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    __del__ = close
+
+    def init_flat(self):
+        self._check(self._lib.kpz_init_flat(self._h))
+
+    def run(self, mcs):
+        self._check(self._lib.kpz_run(self._h, int(mcs)))
+
+    def synchronize(self):
+        self._check(self._lib.kpz_synchronize(self._h))
+
+    def measure(self):
+        """-> (sum_h, sum_h2, W2) numpy arrays of length n_replicas (int64, int64, float64)."""
+        R = self.n_replicas
+        s1 = np.zeros(R, dtype=np.int64)
+        s2 = np.zeros(R, dtype=np.int64)
+        w2 = np.zeros(R, dtype=np.float64)
+        self._check(self._lib.kpz_measure(self._h, s1.ctypes.data, s2.ctypes.data, w2.ctypes.data))
+        return s1, s2, w2
+
+    def get_slopes(self, replica=0):
+        sx = np.zeros((self.L, self.L), dtype=np.int8)
+        sy = np.zeros((self.L, self.L), dtype=np.int8)
+        self._check(self._lib.kpz_get_slopes(self._h, replica, sx.ctypes.data, sy.ctypes.data))
+        return sx, sy
+
+    def get_window(self, x0, y0, w, h, replica=0):
+        sx = np.zeros((h, w), dtype=np.int8)
+        sy = np.zeros((h, w), dtype=np.int8)
+        self._check(self._lib.kpz_get_window(self._h, replica, x0, y0, w, h, sx.ctypes.data, sy.ctypes.data))
+        return sx, sy
+
+    def set_slopes(self, sx, sy, h00=0, replica=0):
+        sx = np.ascontiguousarray(sx, dtype=np.int8)
+        sy = np.ascontiguousarray(sy, dtype=np.int8)
+        if sx.shape != (self.L, self.L) or sy.shape != (self.L, self.L):
+            raise ValueError("slope arrays must be L x L")
+        self._check(self._lib.kpz_set_slopes(self._h, replica, sx.ctypes.data, sy.ctypes.data, int(h00)))
+
+    def state_hash(self, replica=0):
+        out = ctypes.c_uint64()
+        self._check(self._lib.kpz_state_hash(self._h, replica, ctypes.addressof(out)))
+        return out.value
+
+    def counters(self, replica=0):
+        a, d, r, m = (ctypes.c_uint64() for _ in range(4))
+        h = ctypes.c_int64()
+        self._check(self._lib.kpz_counters(self._h, replica, ctypes.addressof(a), ctypes.addressof(d),
+                                           ctypes.addressof(r), ctypes.addressof(h), ctypes.addressof(m)))
+        return {"attempts": a.value, "deposits": d.value, "removals": r.value, "h00": h.value, "mcs": m.value}
+
+    def export_packed(self, host_tensor):
+        self._check(self._lib.kpz_export_packed(self._h, host_tensor.data_ptr(), host_tensor.numel()))
+
+    def import_packed(self, host_tensor, h00=None, mcs=0):
+        h = None if h00 is None else np.ascontiguousarray(h00, dtype=np.int64)
+        self._check(self._lib.kpz_import_packed(self._h, host_tensor.data_ptr(), host_tensor.numel(),
+                                                None if h is None else h.ctypes.data, int(mcs)))
+
+    def step_host(self, host_tensor, h00, mcs_start, mcs):
+        """kpz_step_host: H2D lattice + run + measure + D2H lattice.  h00 (int64 array) is updated in place."""
+        R = self.n_replicas
+        s1 = np.zeros(R, dtype=np.int64)
+        s2 = np.zeros(R, dtype=np.int64)
+        w2 = np.zeros(R, dtype=np.float64)
+        self._check(self._lib.kpz_step_host(self._h, host_tensor.data_ptr(), host_tensor.numel(), h00.ctypes.data,
+                                            int(mcs_start), int(mcs), s1.ctypes.data, s2.ctypes.data, w2.ctypes.data))
+        return s1, s2, w2
+
+    def launch_count(self):
+        out = ctypes.c_uint64()
+        self._check(self._lib.kpz_launch_count(self._h, ctypes.addressof(out)))
+        return out.value

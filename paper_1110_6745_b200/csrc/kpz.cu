@@ -1,0 +1,500 @@
+// kpz.cu -- host side of libkpz_b200.so: the C ABI of include/kpz.h on top of the kernels in kpz_device.cuh.
+// No CPU fallback: every entry point that computes launches CUDA kernels on the bound stream.
+#include "../../include/kpz.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "kpz_device.cuh"
+
+namespace {
+
+typedef __int128 i128;
+typedef unsigned __int128 u128;
+
+struct ScratchLayout {
+    size_t stats;     // [R][4] u64 : deposits, removals, h00, reserved
+    size_t msum;      // [R][4] u64 : lo/hi halves of sum rel, sum rel^2
+    size_t misc;      // 8 x u64    : [0] hash accumulator, [1] validation flags
+    size_t base;      // [R][L] i32
+    size_t cS0;       // [R][NC][L] i32
+    size_t cS1;       // [R][NC][L] i64
+    size_t cS2;       // [R][NC][L] i64
+    size_t total;
+    uint32_t n_chunks, rows_per_chunk;
+};
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+ScratchLayout scratch_layout(uint32_t L, uint32_t R) {
+    ScratchLayout s;
+    const uint32_t W = L / 32, colblocks = (W + 7) / 8;
+    // enough (column block x chunk x replica) CTAs to fill 148 SMs several times; chunks are multiples of 32 rows
+    uint64_t want = 148ull * 8ull;
+    uint64_t have = (uint64_t)colblocks * R;
+    uint32_t nc = (uint32_t)((want + have - 1) / have);
+    uint32_t max_nc = L / 32;
+    if (nc > max_nc) nc = max_nc;
+    if (nc < 1) nc = 1;
+    uint32_t rpc = (L + nc - 1) / nc;
+    rpc = (rpc + 31) / 32 * 32;
+    nc = (L + rpc - 1) / rpc;
+    s.n_chunks = nc;
+    s.rows_per_chunk = rpc;
+    size_t o = 0;
+    s.stats = o; o += align_up((size_t)R * 4 * 8, 256);
+    s.msum = o;  o += align_up((size_t)R * 4 * 8, 256);
+    s.misc = o;  o += 256;
+    s.base = o;  o += align_up((size_t)R * L * 4, 256);
+    s.cS0 = o;   o += align_up((size_t)R * nc * L * 4, 256);
+    s.cS1 = o;   o += align_up((size_t)R * nc * L * 8, 256);
+    s.cS2 = o;   o += align_up((size_t)R * nc * L * 8, 256);
+    s.total = o;
+    return s;
+}
+
+bool valid_tile(uint32_t T) { return T == 4 || T == 8 || T == 16 || T == 32 || T == 64; }
+
+int32_t validate(uint32_t L, double p, double q, uint32_t T, uint32_t R) {
+    if (!valid_tile(T)) return KPZ_EINVAL;
+    if (L == 0 || L % (2 * T) != 0 || L % 32 != 0) return KPZ_EINVAL;
+    if (!(p >= 0.0 && p <= 1.0) || !(q >= 0.0 && q <= 1.0)) return KPZ_EINVAL;
+    if (R == 0) return KPZ_EINVAL;
+    if (L > (1u << 20)) return KPZ_EINVAL;   // int32 heights / tile ids stay in range up to 2^20
+    const uint64_t NT = L / T;
+    if (NT * NT >= 0xFFFFFFFFull) return KPZ_EINVAL;   // tile_id must never equal the global-draw marker
+    return KPZ_OK;
+}
+
+uint64_t accept_threshold(double prob) {
+    if (prob >= 1.0) return 1ull << 32;
+    if (prob <= 0.0) return 0ull;
+    return (uint64_t)std::floor(std::ldexp(prob, 32));
+}
+
+}  // namespace
+
+struct kpz_ctx {
+    uint32_t L, T, R;
+    double p, q;
+    uint64_t seed;
+    uint64_t mcs;            // completed MCS (all replicas advance together)
+    uint64_t launches;
+    uint32_t* d_lattice;
+    unsigned char* d_scratch;
+    cudaStream_t stream;
+    bool bound;
+    ScratchLayout sl;
+    size_t lattice_bytes;
+    int max_smem_optin;
+    char err[512];
+};
+
+namespace {
+
+int32_t fail(kpz_ctx* c, int32_t code, const char* fmt, ...) {
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define KPZ_CUDA(c, expr)                                                                          \
+    do {                                                                                           \
+        cudaError_t e__ = (expr);                                                                  \
+        if (e__ != cudaSuccess)                                                                    \
+            return fail((c), KPZ_ECUDA, "%s failed: %s", #expr, cudaGetErrorString(e__));          \
+    } while (0)
+
+int grid_for(uint64_t n, int block, int cap = 148 * 16) {
+    uint64_t g = (n + block - 1) / block;
+    if (g > (uint64_t)cap) g = cap;
+    if (g < 1) g = 1;
+    return (int)g;
+}
+
+template <int T, int NTHR, int MODE>
+int32_t launch_update_t(kpz_ctx* c, const kpz::UpdateParams& P) {
+    const size_t smem = (size_t)kpz::TileGeom<T>::WORDS * NTHR * sizeof(uint32_t);
+    auto kern = kpz::kpz_update_kernel<T, NTHR, MODE>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        KPZ_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        KPZ_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        attr_set = true;
+    }
+    const uint64_t blocks = (P.total_items + NTHR - 1) / NTHR;
+    if (blocks > 0x7FFFFFFFull) return fail(c, KPZ_EINVAL, "too many tiles for one launch");
+    kern<<<(unsigned)blocks, NTHR, smem, c->stream>>>(P);
+    KPZ_CUDA(c, cudaGetLastError());
+    c->launches++;
+    return KPZ_OK;
+}
+
+template <int T, int NTHR>
+int32_t launch_update_mode(kpz_ctx* c, const kpz::UpdateParams& P) {
+    const bool simple = (c->p >= 1.0 && c->q <= 0.0);
+    return simple ? launch_update_t<T, NTHR, 0>(c, P) : launch_update_t<T, NTHR, 1>(c, P);
+}
+
+int32_t launch_update(kpz_ctx* c, uint32_t m, uint32_t slot) {
+    kpz::UpdateParams P;
+    P.lattice = c->d_lattice;
+    P.stats = reinterpret_cast<unsigned long long*>(c->d_scratch + c->sl.stats);
+    P.plane_words = (uint64_t)c->L * c->L / 32;
+    P.L = c->L;
+    P.NT = c->L / c->T;
+    P.HN = P.NT / 2;
+    P.W = c->L / 32;
+    P.tiles_per_colour = P.HN * P.HN;
+    P.total_items = (uint64_t)c->R * P.tiles_per_colour;
+    P.blocked = (P.HN % 8 == 0) ? 1u : 0u;
+    P.thr_p = accept_threshold(c->p);
+    P.thr_q = accept_threshold(c->q);
+    P.m = m;
+    P.slot = slot;
+    P.key.k0 = (uint32_t)(c->seed & 0xFFFFFFFFull);
+    P.key.k1 = (uint32_t)(c->seed >> 32);
+    switch (c->T) {
+        case 64: return launch_update_mode<64, 32>(c, P);
+        case 32: return launch_update_mode<32, 64>(c, P);
+        case 16: return launch_update_mode<16, 128>(c, P);
+        case 8: return launch_update_mode<8, 128>(c, P);
+        case 4: return launch_update_mode<4, 128>(c, P);
+    }
+    return fail(c, KPZ_EINVAL, "unsupported tile %u", c->T);
+}
+
+int32_t require_bound(kpz_ctx* c) {
+    if (!c) return KPZ_EINVAL;
+    if (!c->bound) return fail(c, KPZ_ESTATE, "kpz_bind has not been called");
+    return KPZ_OK;
+}
+
+// sums for all replicas -> host vectors (relative to h(0,0)) + h00
+int32_t measure_relative(kpz_ctx* c, std::vector<i128>& S1, std::vector<i128>& S2, std::vector<long long>& h00) {
+    const uint32_t L = c->L, R = c->R, W = L / 32;
+    const uint64_t plane_words = (uint64_t)L * L / 32;
+    unsigned char* sc = c->d_scratch;
+    unsigned long long* msum = reinterpret_cast<unsigned long long*>(sc + c->sl.msum);
+    int32_t* base = reinterpret_cast<int32_t*>(sc + c->sl.base);
+    int32_t* cS0 = reinterpret_cast<int32_t*>(sc + c->sl.cS0);
+    long long* cS1 = reinterpret_cast<long long*>(sc + c->sl.cS1);
+    long long* cS2 = reinterpret_cast<long long*>(sc + c->sl.cS2);
+    KPZ_CUDA(c, cudaMemsetAsync(msum, 0, (size_t)R * 32, c->stream));
+    int nthr = 1024;
+    while (nthr > 32 && (uint32_t)nthr > L) nthr >>= 1;
+    kpz::kpz_row0_prefix_kernel<<<R, nthr, 0, c->stream>>>(c->d_lattice, plane_words, L, W, base);
+    KPZ_CUDA(c, cudaGetLastError());
+    dim3 g1((W + 7) / 8, c->sl.n_chunks, R);
+    kpz::kpz_column_chunk_kernel<<<g1, 256, 0, c->stream>>>(c->d_lattice, plane_words, L, W, c->sl.rows_per_chunk, cS0,
+                                                         cS1, cS2);
+    KPZ_CUDA(c, cudaGetLastError());
+    dim3 g2((L + 255) / 256, R);
+    kpz::kpz_combine_kernel<<<g2, 256, 0, c->stream>>>(base, cS0, cS1, cS2, L, c->sl.n_chunks, c->sl.rows_per_chunk, msum);
+    KPZ_CUDA(c, cudaGetLastError());
+    c->launches += 3;
+    std::vector<unsigned long long> hm((size_t)R * 4), hs((size_t)R * 4);
+    KPZ_CUDA(c, cudaMemcpyAsync(hm.data(), msum, (size_t)R * 32, cudaMemcpyDeviceToHost, c->stream));
+    KPZ_CUDA(c, cudaMemcpyAsync(hs.data(), sc + c->sl.stats, (size_t)R * 32, cudaMemcpyDeviceToHost, c->stream));
+    KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
+    S1.resize(R); S2.resize(R); h00.resize(R);
+    for (uint32_t r = 0; r < R; ++r) {
+        S1[r] = (i128)(long long)hm[4 * r + 1] * ((i128)1 << 32) + (i128)hm[4 * r + 0];
+        S2[r] = (i128)(long long)hm[4 * r + 3] * ((i128)1 << 32) + (i128)hm[4 * r + 2];
+        h00[r] = (long long)hs[4 * r + 2];
+    }
+    return KPZ_OK;
+}
+
+bool fits_i64(i128 v) { return v >= (i128)INT64_MIN && v <= (i128)INT64_MAX; }
+
+}  // namespace
+
+extern "C" {
+
+int32_t kpz_workspace_bytes(uint32_t L, uint32_t tile, uint32_t n_replicas, size_t* lattice_bytes,
+                            size_t* scratch_bytes) {
+    int32_t rc = validate(L, 0.0, 0.0, tile, n_replicas);
+    if (rc != KPZ_OK) return rc;
+    if (lattice_bytes) *lattice_bytes = (size_t)n_replicas * ((size_t)L * L / 4);
+    if (scratch_bytes) *scratch_bytes = scratch_layout(L, n_replicas).total;
+    return KPZ_OK;
+}
+
+int32_t kpz_create_batch(kpz_ctx** out, uint32_t L, double p, double q, uint32_t tile, uint64_t seed,
+                         uint32_t n_replicas) {
+    if (!out) return KPZ_EINVAL;
+    *out = nullptr;
+    int32_t rc = validate(L, p, q, tile, n_replicas);
+    if (rc != KPZ_OK) return rc;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0) return KPZ_ECUDA;   // no CPU fallback
+    kpz_ctx* c = new (std::nothrow) kpz_ctx();
+    if (!c) return KPZ_ENOMEM;
+    c->L = L; c->T = tile; c->R = n_replicas; c->p = p; c->q = q; c->seed = seed;
+    c->mcs = 0; c->launches = 0;
+    c->d_lattice = nullptr; c->d_scratch = nullptr; c->stream = nullptr; c->bound = false;
+    c->sl = scratch_layout(L, n_replicas);
+    c->lattice_bytes = (size_t)n_replicas * ((size_t)L * L / 4);
+    c->err[0] = 0;
+    *out = c;
+    return KPZ_OK;
+}
+
+int32_t kpz_create(kpz_ctx** out, uint32_t L, double p, double q, uint32_t tile, uint64_t seed) {
+    return kpz_create_batch(out, L, p, q, tile, seed, 1);
+}
+
+int32_t kpz_bind(kpz_ctx* c, void* d_lattice, size_t lattice_bytes, void* d_scratch, size_t scratch_bytes,
+                 void* cuda_stream) {
+    if (!c) return KPZ_EINVAL;
+    if (!d_lattice || !d_scratch) return fail(c, KPZ_EINVAL, "NULL device buffer");
+    if (lattice_bytes < c->lattice_bytes || scratch_bytes < c->sl.total)
+        return fail(c, KPZ_ENOMEM, "bound buffers too small: need %zu + %zu bytes", c->lattice_bytes, c->sl.total);
+    if (((uintptr_t)d_lattice & 15u) || ((uintptr_t)d_scratch & 15u)) return fail(c, KPZ_EINVAL, "buffers must be 16-byte aligned");
+    c->d_lattice = static_cast<uint32_t*>(d_lattice);
+    c->d_scratch = static_cast<unsigned char*>(d_scratch);
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    KPZ_CUDA(c, cudaMemsetAsync(c->d_scratch, 0, c->sl.base, c->stream));   // counters, sums, misc
+    c->bound = true;
+    return KPZ_OK;
+}
+
+int32_t kpz_init_flat(kpz_ctx* c) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    const uint64_t n_words = (uint64_t)c->R * ((uint64_t)c->L * c->L / 16);
+    kpz::kpz_fill_flat_kernel<<<grid_for(n_words, 256, 148 * 32), 256, 0, c->stream>>>(c->d_lattice, n_words, c->L / 32);
+    KPZ_CUDA(c, cudaGetLastError());
+    c->launches++;
+    KPZ_CUDA(c, cudaMemsetAsync(c->d_scratch + c->sl.stats, 0, (size_t)c->R * 32, c->stream));
+    c->mcs = 0;
+    return KPZ_OK;
+}
+
+int32_t kpz_run(kpz_ctx* c, uint64_t mcs) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    if (c->mcs + mcs > 0xFFFFFFFFull) return fail(c, KPZ_EINVAL, "MCS clock would exceed 2^32-1");
+    for (uint64_t k = 0; k < mcs; ++k) {
+        const uint32_t m = (uint32_t)c->mcs;
+        for (uint32_t slot = 0; slot < 4; ++slot) {
+            rc = launch_update(c, m, slot);
+            if (rc != KPZ_OK) return rc;
+        }
+        c->mcs++;
+    }
+    return KPZ_OK;
+}
+
+int32_t kpz_measure(kpz_ctx* c, int64_t* sum_h, int64_t* sum_h2, double* W2) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    std::vector<i128> S1, S2;
+    std::vector<long long> h00;
+    rc = measure_relative(c, S1, S2, h00);
+    if (rc != KPZ_OK) return rc;
+    const i128 N = (i128)c->L * c->L;
+    const double Nd = (double)((uint64_t)c->L * c->L);
+    bool overflow = false;
+    for (uint32_t r = 0; r < c->R; ++r) {
+        const i128 h0 = h00[r];
+        const i128 sh = S1[r] + N * h0;                          // sum h
+        const i128 sh2 = S2[r] + 2 * h0 * S1[r] + N * h0 * h0;   // sum h^2
+        // N*sum_h2 - sum_h^2 is invariant under the shift by h0: evaluate it on the small relative sums
+        const i128 num = N * S2[r] - S1[r] * S1[r];
+        if (W2) W2[r] = (double)num / (Nd * Nd);
+        if (sum_h) { if (fits_i64(sh)) sum_h[r] = (int64_t)sh; else { sum_h[r] = 0; overflow = true; } }
+        if (sum_h2) { if (fits_i64(sh2)) sum_h2[r] = (int64_t)sh2; else { sum_h2[r] = 0; overflow = true; } }
+    }
+    if (overflow) return fail(c, KPZ_EOVERFLOW, "a sum does not fit int64");
+    return KPZ_OK;
+}
+
+int32_t kpz_destroy(kpz_ctx* c) {
+    delete c;
+    return KPZ_OK;
+}
+
+int32_t kpz_synchronize(kpz_ctx* c) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
+    return KPZ_OK;
+}
+
+const char* kpz_last_error(const kpz_ctx* c) { return c ? c->err : "null handle"; }
+
+int32_t kpz_get_window(kpz_ctx* c, uint32_t replica, uint32_t x0, uint32_t y0, uint32_t w, uint32_t h, int8_t* sx,
+                       int8_t* sy) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    if (replica >= c->R || !sx || !sy || w == 0 || h == 0 || w > c->L || h > c->L) return fail(c, KPZ_EINVAL, "bad window");
+    const size_t n = (size_t)w * h;
+    int8_t* d = nullptr;
+    if (cudaMalloc(&d, 2 * n) != cudaSuccess) { cudaGetLastError(); return fail(c, KPZ_ENOMEM, "temporary device buffer"); }
+    kpz::kpz_unpack_window_kernel<<<grid_for(n, 256), 256, 0, c->stream>>>(c->d_lattice, (uint64_t)c->L * c->L / 32, replica,
+                                                                       c->L, c->L / 32, x0 % c->L, y0 % c->L, w, h, d, d + n);
+    cudaError_t e = cudaGetLastError();
+    c->launches++;
+    if (e == cudaSuccess) e = cudaMemcpyAsync(sx, d, n, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(sy, d + n, n, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    cudaFree(d);
+    if (e != cudaSuccess) return fail(c, KPZ_ECUDA, "get_window: %s", cudaGetErrorString(e));
+    return KPZ_OK;
+}
+
+int32_t kpz_get_slopes(kpz_ctx* c, uint32_t replica, int8_t* sx, int8_t* sy) {
+    if (!c) return KPZ_EINVAL;
+    return kpz_get_window(c, replica, 0, 0, c->L, c->L, sx, sy);
+}
+
+int32_t kpz_set_slopes(kpz_ctx* c, uint32_t replica, const int8_t* sx, const int8_t* sy, int64_t h00) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    if (replica >= c->R || !sx || !sy) return fail(c, KPZ_EINVAL, "bad argument");
+    const size_t n = (size_t)c->L * c->L;
+    int8_t* d = nullptr;
+    if (cudaMalloc(&d, 2 * n) != cudaSuccess) { cudaGetLastError(); return fail(c, KPZ_ENOMEM, "temporary device buffer"); }
+    int* flags = reinterpret_cast<int*>(c->d_scratch + c->sl.misc + 8);
+    int hflags = 0;
+    cudaError_t e = cudaMemcpyAsync(d, sx, n, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d + n, sy, n, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(flags, 0, sizeof(int), c->stream);
+    if (e == cudaSuccess) {
+        kpz::kpz_validate_kernel<<<grid_for(n, 256), 256, 0, c->stream>>>(d, d + n, c->L, flags);
+        c->launches++;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&hflags, flags, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e == cudaSuccess && hflags == 0) {
+        kpz::kpz_pack_kernel<<<grid_for(n / 32, 256), 256, 0, c->stream>>>(c->d_lattice, (uint64_t)n / 32, replica, c->L,
+                                                                      c->L / 32, d, d + n);
+        c->launches++;
+        e = cudaGetLastError();
+        long long hv = h00;
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(c->d_scratch + c->sl.stats + (size_t)replica * 32 + 16, &hv, 8, cudaMemcpyHostToDevice, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    }
+    cudaFree(d);
+    if (e != cudaSuccess) return fail(c, KPZ_ECUDA, "set_slopes: %s", cudaGetErrorString(e));
+    if (hflags & 1) return fail(c, KPZ_EINVAL, "slopes must be +1 or -1");
+    if (hflags) return fail(c, KPZ_ESTATE, "state is not curl-free with zero tilt (flags %d)", hflags);
+    return KPZ_OK;
+}
+
+int32_t kpz_state_hash(kpz_ctx* c, uint32_t replica, uint64_t* out) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    if (replica >= c->R || !out) return fail(c, KPZ_EINVAL, "bad argument");
+    unsigned long long* acc = reinterpret_cast<unsigned long long*>(c->d_scratch + c->sl.misc);
+    const uint64_t plane_words = (uint64_t)c->L * c->L / 32;
+    KPZ_CUDA(c, cudaMemsetAsync(acc, 0, 8, c->stream));
+    kpz::kpz_hash_kernel<<<grid_for(plane_words, 256), 256, 0, c->stream>>>(c->d_lattice, plane_words, replica, c->L, c->L / 32, acc);
+    KPZ_CUDA(c, cudaGetLastError());
+    c->launches++;
+    unsigned long long h = 0;
+    KPZ_CUDA(c, cudaMemcpyAsync(&h, acc, 8, cudaMemcpyDeviceToHost, c->stream));
+    KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
+    *out = h;
+    return KPZ_OK;
+}
+
+int32_t kpz_counters(kpz_ctx* c, uint32_t replica, uint64_t* attempts, uint64_t* deposits, uint64_t* removals,
+                     int64_t* h00, uint64_t* mcs) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    if (replica >= c->R) return fail(c, KPZ_EINVAL, "replica out of range");
+    unsigned long long st[4];
+    KPZ_CUDA(c, cudaMemcpyAsync(st, c->d_scratch + c->sl.stats + (size_t)replica * 32, 32, cudaMemcpyDeviceToHost, c->stream));
+    KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (attempts) *attempts = c->mcs * (uint64_t)c->L * c->L;
+    if (deposits) *deposits = st[0];
+    if (removals) *removals = st[1];
+    if (h00) *h00 = (int64_t)st[2];
+    if (mcs) *mcs = c->mcs;
+    return KPZ_OK;
+}
+
+int32_t kpz_export_packed(kpz_ctx* c, void* host_dst, size_t bytes) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    if (!host_dst || bytes < c->lattice_bytes) return fail(c, KPZ_EINVAL, "host buffer too small");
+    KPZ_CUDA(c, cudaMemcpyAsync(host_dst, c->d_lattice, c->lattice_bytes, cudaMemcpyDeviceToHost, c->stream));
+    KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
+    return KPZ_OK;
+}
+
+int32_t kpz_import_packed(kpz_ctx* c, const void* host_src, size_t bytes, const int64_t* h00, uint64_t mcs) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    if (!host_src || bytes < c->lattice_bytes || mcs > 0xFFFFFFFFull) return fail(c, KPZ_EINVAL, "bad argument");
+    KPZ_CUDA(c, cudaMemcpyAsync(c->d_lattice, host_src, c->lattice_bytes, cudaMemcpyHostToDevice, c->stream));
+    std::vector<unsigned long long> st((size_t)c->R * 4, 0ull);
+    KPZ_CUDA(c, cudaMemcpyAsync(st.data(), c->d_scratch + c->sl.stats, (size_t)c->R * 32, cudaMemcpyDeviceToHost, c->stream));
+    KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (uint32_t r = 0; r < c->R; ++r) st[4 * r + 2] = (unsigned long long)(h00 ? h00[r] : 0);
+    KPZ_CUDA(c, cudaMemcpyAsync(c->d_scratch + c->sl.stats, st.data(), (size_t)c->R * 32, cudaMemcpyHostToDevice, c->stream));
+    KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->mcs = mcs;
+    return KPZ_OK;
+}
+
+int32_t kpz_step_host(kpz_ctx* c, void* host_lattice, size_t bytes, int64_t* h00_inout, uint64_t mcs_start, uint64_t mcs,
+                      int64_t* sum_h, int64_t* sum_h2, double* W2) {
+    int32_t rc = kpz_import_packed(c, host_lattice, bytes, h00_inout, mcs_start);
+    if (rc != KPZ_OK) return rc;
+    rc = kpz_run(c, mcs);
+    if (rc != KPZ_OK) return rc;
+    rc = kpz_measure(c, sum_h, sum_h2, W2);
+    if (rc != KPZ_OK && rc != KPZ_EOVERFLOW) return rc;
+    int32_t rc2 = kpz_export_packed(c, host_lattice, bytes);
+    if (rc2 != KPZ_OK) return rc2;
+    if (h00_inout) {
+        for (uint32_t r = 0; r < c->R; ++r) {
+            int64_t h;
+            rc2 = kpz_counters(c, r, nullptr, nullptr, nullptr, &h, nullptr);
+            if (rc2 != KPZ_OK) return rc2;
+            h00_inout[r] = h;
+        }
+    }
+    return rc;
+}
+
+int32_t kpz_launch_count(const kpz_ctx* c, uint64_t* out) {
+    if (!c || !out) return KPZ_EINVAL;
+    *out = c->launches;
+    return KPZ_OK;
+}
+
+int32_t kpz_philox_selftest(const uint32_t* ctr, const uint32_t* key, uint32_t* out, uint32_t n) {
+    if (!ctr || !key || !out || n == 0) return KPZ_EINVAL;
+    uint32_t *dc = nullptr, *dk = nullptr, *dout = nullptr;
+    if (cudaMalloc(&dc, 16 * (size_t)n) != cudaSuccess) { cudaGetLastError(); return KPZ_ECUDA; }
+    if (cudaMalloc(&dk, 8 * (size_t)n) != cudaSuccess) { cudaGetLastError(); cudaFree(dc); return KPZ_ECUDA; }
+    if (cudaMalloc(&dout, 16 * (size_t)n) != cudaSuccess) { cudaGetLastError(); cudaFree(dc); cudaFree(dk); return KPZ_ECUDA; }
+    cudaError_t e = cudaMemcpy(dc, ctr, 16 * (size_t)n, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(dk, key, 8 * (size_t)n, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        kpz::kpz_philox_selftest_kernel<<<(n + 127) / 128, 128>>>(dc, dk, dout, n);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(out, dout, 16 * (size_t)n, cudaMemcpyDeviceToHost);
+    cudaFree(dc); cudaFree(dk); cudaFree(dout);
+    return e == cudaSuccess ? KPZ_OK : KPZ_ECUDA;
+}
+
+}  // extern "C"

@@ -1,0 +1,318 @@
+"""GPU parity tests proper: the CUDA path (through the C ABI) vs the CPU oracle, element by element, bit-exact.
+Tolerance: 0 for the lattice state, the int64 sums and W^2 (derived in double from exact integers)."""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import Oracle
+import oracle as oracle_mod
+import kpz_inputs as gen
+
+pytestmark = pytest.mark.gpu
+
+NTHREADS = max(1, min(32, os.cpu_count() or 1))
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    import __graft_entry__ as g
+    g.build()
+    import paper_1110_6745_b200 as pkg
+    return pkg
+
+
+def _kat():
+    from pathlib import Path
+    rows = []
+    for line in (Path(__file__).parent / "golden" / "philox4x32_10_kat.txt").read_text().splitlines():
+        if line.startswith("#") or not line.strip():
+            continue
+        v = [int(t, 16) for t in line.split()]
+        rows.append(v)
+    return np.array(rows, dtype=np.uint64)
+
+
+def test_device_philox_known_answers(pkg):
+    k = _kat()
+    out = pkg.philox_selftest(k[:, 0:4].astype(np.uint32), k[:, 4:6].astype(np.uint32))
+    assert np.array_equal(out, k[:, 6:10].astype(np.uint32))
+    rng = np.random.default_rng(0)
+    ctr = rng.integers(0, 2**32, size=(257, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2**32, size=(257, 2), dtype=np.uint64).astype(np.uint32)
+    out = pkg.philox_selftest(ctr, key)
+    for i in range(0, 257, 16):
+        assert np.array_equal(out[i], oracle_mod.philox4x32_10(ctr[i], key[i]))
+
+
+@pytest.mark.parametrize("L,T", [(32, 4), (64, 8), (256, 16), (128, 64), (4096, 32), (96, 16)])
+def test_flat_init(pkg, L, T):
+    k = pkg.KPZ(L, 1.0, 0.0, T, 1)
+    k.init_flat()
+    s1, s2, w2 = k.measure()
+    assert s1[0] == L * L // 2 and s2[0] == L * L // 2 and w2[0] == 0.25
+    if L <= 256:
+        sx, sy = k.get_slopes()
+        ex, ey = gen.heights_to_slopes(gen.flat_heights(L))
+        assert np.array_equal(sx, ex) and np.array_equal(sy, ey)
+    o = Oracle(L, 1.0, 0.0, T, 1)
+    o.init_flat()
+    assert k.state_hash() == o.state_hash()
+    c = k.counters()
+    assert c == {"attempts": 0, "deposits": 0, "removals": 0, "h00": 0, "mcs": 0}
+
+
+@pytest.mark.parametrize("L,kind", [(64, "tri1"), (64, "tri8"), (256, "raised"), (128, "stair"), (96, "raised"),
+                                    (1024, "raised"), (2048, "stair")])
+def test_measure_pack_unpack_hash_parity(pkg, L, kind):
+    if kind == "tri1":
+        h = gen.triangle_heights(L, 1)
+    elif kind == "tri8":
+        h = gen.triangle_heights(L, 8)
+    elif kind == "raised":
+        h = gen.raised_flat_heights(L, 11, 0.4) - 5
+    else:
+        h = gen.staircase_heights(L, 3) + 3_000_000_000
+    sx, sy = gen.heights_to_slopes(h)
+    k = pkg.KPZ(L, 1.0, 0.0, 16, 1)
+    k.init_flat()
+    k.set_slopes(sx, sy, h00=int(h[0, 0]))
+    gx, gy = k.get_slopes()
+    assert np.array_equal(gx, sx) and np.array_equal(gy, sy)
+    o = Oracle(L, 1.0, 0.0, 16, 1)
+    o.set_slopes(sx, sy, h00=int(h[0, 0]))
+    s1, s2, w2 = k.measure()
+    os1, os2, ow2 = o.measure()
+    assert int(s1[0]) == os1 == int(h.sum())
+    assert int(s2[0]) == os2
+    assert float(w2[0]) == ow2
+    assert k.state_hash() == o.state_hash()
+    if kind == "tri8":
+        assert abs(w2[0] - (64 + 2) / 6) < 1e-12
+    # window with wrap
+    wx, wy = k.get_window(L - 5, L - 3, 17, 9)
+    ys = (L - 3 + np.arange(9)) % L
+    xs = (L - 5 + np.arange(17)) % L
+    assert np.array_equal(wx, sx[np.ix_(ys, xs)]) and np.array_equal(wy, sy[np.ix_(ys, xs)])
+
+
+def test_measure_overflow_and_set_slopes_validation(pkg):
+    L = 64
+    k = pkg.KPZ(L, 1.0, 0.0, 16, 1)
+    k.init_flat()
+    h = gen.flat_heights(L)
+    sx, sy = gen.heights_to_slopes(h)
+    k.set_slopes(sx, sy, h00=2**62)                       # sum h overflows int64
+    with pytest.raises(pkg.KpzError) as e:
+        k.measure()
+    assert e.value.code == pkg.KPZ_EOVERFLOW
+    bad = sx.copy(); bad[3, 3] = 0
+    with pytest.raises(pkg.KpzError) as e:
+        k.set_slopes(bad, sy)
+    assert e.value.code == pkg.KPZ_EINVAL
+    bad = sx.copy(); bad[3, 3] = -bad[3, 3]               # breaks curl-free / zero tilt
+    with pytest.raises(pkg.KpzError) as e:
+        k.set_slopes(bad, sy)
+    assert e.value.code == pkg.KPZ_ESTATE
+    k.set_slopes(sx, sy, h00=0)
+    assert k.measure()[2][0] == 0.25
+
+
+def _compare_full(k, o, replica=0):
+    sx, sy = k.get_slopes(replica)
+    osx, osy = o.slopes()
+    assert np.array_equal(sx, osx), "sigma_x differs at %d sites" % int((sx != osx).sum())
+    assert np.array_equal(sy, osy), "sigma_y differs at %d sites" % int((sy != osy).sum())
+
+
+def _compare_scalars(k, os_, replica_slice=None):
+    s1, s2, w2 = k.measure()
+    for r, o in enumerate(os_):
+        os1, os2, ow2 = o.measure()
+        assert int(s1[r]) == os1 and int(s2[r]) == os2, (r, int(s1[r]), os1, int(s2[r]), os2)
+        assert float(w2[r]) == ow2
+        c, oc = k.counters(r), o.counters()
+        assert c == oc, (c, oc)
+
+
+@pytest.mark.parametrize("L,T,p,q,seed,n", [
+    (32, 4, 1.0, 0.0, 1, 6),
+    (64, 8, 0.75, 0.25, 2, 6),
+    (64, 16, 1.0, 0.0, 3, 8),
+    (96, 16, 0.5, 0.5, 4, 5),          # L not a power of two
+    (128, 32, 1.0, 0.0, 5, 6),
+    (128, 64, 0.75, 0.25, 6, 6),       # a single tile per colour
+    (192, 32, 0.3, 0.9, 7, 4),
+    (384, 64, 1.0, 0.0, 2**40 + 17, 5),
+    (512, 64, 0.75, 0.25, 9, 5),       # blocked lane mapping needs HN % 8 == 0: HN = 4 -> linear
+    (1024, 64, 1.0, 0.0, 10, 4),       # HN = 8 -> blocked lane mapping
+    (1024, 32, 0.6, 0.1, 11, 3),
+    (1024, 16, 1.0, 0.0, 12, 3),
+])
+def test_update_parity_every_mcs(pkg, L, T, p, q, seed, n):
+    k = pkg.KPZ(L, p, q, T, seed)
+    k.init_flat()
+    o = Oracle(L, p, q, T, seed, threads=NTHREADS)
+    o.init_flat()
+    for t in range(n):
+        k.run(1)
+        o.run(1)
+        _compare_full(k, o)
+        _compare_scalars(k, [o])
+        assert k.state_hash() == o.state_hash()
+
+
+def test_config1_full(pkg):
+    """BASELINE config 1: L=256, T=16, p=1, q=0, seed 1, 64 MCS; state and sums after EVERY MCS."""
+    L, T, seed = 256, 16, 1
+    k = pkg.KPZ(L, 1.0, 0.0, T, seed)
+    k.init_flat()
+    o = Oracle(L, 1.0, 0.0, T, seed)
+    o.init_flat()
+    w2_series = {}
+    for t in range(1, 65):
+        k.run(1); o.run(1)
+        _compare_full(k, o)
+        _compare_scalars(k, [o])
+        if t in (1, 2, 4, 8, 16, 32, 64):
+            w2_series[t] = float(k.measure()[2][0])
+    assert all(w2_series[a] < w2_series[b] for a, b in zip((1, 2, 4, 8, 16, 32), (2, 4, 8, 16, 32, 64)))
+    assert 1.5 < w2_series[64] < 2.8          # ~2.08 +- ensemble spread at L=256, T=16
+
+
+CONFIG2_TIMES = [1, 2, 3, 4, 5, 7, 9, 11, 14, 17, 22, 28, 36, 45, 57, 73, 92, 117, 149, 189, 240, 304, 386, 489,
+                 621, 788, 1000]
+
+
+def test_config2_prefix(pkg):
+    """BASELINE config 2: L=4096, T=32, p=1, q=0, seed 7; the log-spaced sample times up to KPZ_CONFIG2_TMAX
+    (default 45; 1000 = the whole config) with the full state compared at every sample."""
+    tmax = int(os.environ.get("KPZ_CONFIG2_TMAX", "45"))
+    L, T, seed = 4096, 32, 7
+    k = pkg.KPZ(L, 1.0, 0.0, T, seed)
+    k.init_flat()
+    o = Oracle(L, 1.0, 0.0, T, seed, threads=NTHREADS)
+    o.init_flat()
+    t = 0
+    for ts in [x for x in CONFIG2_TIMES if x <= tmax]:
+        k.run(ts - t); o.run(ts - t)
+        t = ts
+        _compare_scalars(k, [o])
+        assert k.state_hash() == o.state_hash()
+    _compare_full(k, o)
+
+
+def test_replica_batch_parity(pkg):
+    """Config-4 shape: independent replicas of L=128, T=16, p=1, q=0, seed 4 (replica id = Philox counter word)."""
+    L, T, seed, R, n = 128, 16, 4, 48, 12
+    k = pkg.KPZ(L, 1.0, 0.0, T, seed, n_replicas=R)
+    k.init_flat()
+    os_ = [Oracle(L, 1.0, 0.0, T, seed, replica=r) for r in range(R)]
+    for o in os_:
+        o.init_flat(); o.run(n)
+    k.run(n)
+    _compare_scalars(k, os_)
+    for r in (0, 1, 17, R - 1):
+        _compare_full(k, os_[r], replica=r)
+        assert k.state_hash(r) == os_[r].state_hash()
+    assert len({k.state_hash(r) for r in range(R)}) == R
+
+
+def test_replica_batch_1024_general_pq(pkg):
+    L, T, seed, R, n = 128, 16, 4, 1024, 3
+    k = pkg.KPZ(L, 0.75, 0.25, T, seed, n_replicas=R)
+    k.init_flat()
+    k.run(n)
+    s1, s2, w2 = k.measure()
+    for r in (0, 5, 511, 1023):
+        o = Oracle(L, 0.75, 0.25, T, seed, replica=r)
+        o.init_flat(); o.run(n)
+        assert (int(s1[r]), int(s2[r]), float(w2[r])) == o.measure()
+        assert k.state_hash(r) == o.state_hash()
+        assert k.counters(r) == o.counters()
+
+
+def test_run_split_checkpoint_and_step_host(pkg):
+    import torch
+    L, T, seed = 512, 32, 77
+    a = pkg.KPZ(L, 0.75, 0.25, T, seed)
+    b = pkg.KPZ(L, 0.75, 0.25, T, seed)
+    a.init_flat(); b.init_flat()
+    a.run(7)
+    b.run(3)
+    host = torch.empty(b.lattice_bytes, dtype=torch.uint8).pin_memory()
+    b.export_packed(host)
+    h00 = np.array([b.counters()["h00"]], dtype=np.int64)
+    c = pkg.KPZ(L, 0.75, 0.25, T, seed)
+    s1, s2, w2 = c.step_host(host, h00, 3, 4)       # resume at MCS 3, run 4 more, through HOST buffers
+    assert a.state_hash() == c.state_hash()
+    assert (int(a.measure()[0][0]), int(a.measure()[1][0])) == (int(s1[0]), int(s2[0]))
+    assert h00[0] == a.counters()["h00"]
+    b.run(4)
+    assert a.state_hash() == b.state_hash()
+    host2 = torch.empty(b.lattice_bytes, dtype=torch.uint8).pin_memory()
+    b.export_packed(host2)
+    assert torch.equal(host, host2)                 # step_host wrote the advanced lattice back
+
+
+def _window_check(pkg, k, L, T, p, q, seed, n_mcs, wx0, wy0, W, check_h00=False):
+    M = 4 * (T + 1) * n_mcs
+    full = W + 2 * M
+    o = Oracle(L, p, q, T, seed, window=((wx0 - M) % L, (wy0 - M) % L, full, full), threads=NTHREADS)
+    o.init_flat(); o.run(n_mcs)
+    osx, osy = o.slopes()
+    gx, gy = k.get_window(wx0, wy0, W, W)
+    assert np.array_equal(gx, osx[M:M + W, M:M + W]), (wx0, wy0)
+    assert np.array_equal(gy, osy[M:M + W, M:M + W]), (wx0, wy0)
+    if check_h00:
+        assert k.counters()["h00"] == o.counters()["h00"]
+
+
+def test_config3_full_size_windows_and_invariants(pkg):
+    """BASELINE config 3 at full size (L=2^17, T=64, p=1, q=0, seed 42), in the launch configuration bench.py
+    times: sampled windows vs the light-cone window oracle + properties that hold at any size."""
+    import torch
+    torch.cuda.empty_cache()
+    L, T, seed, n = 1 << 17, 64, 42, 2
+    k = pkg.KPZ(L, 1.0, 0.0, T, seed)
+    k.init_flat()
+    k.run(n)
+    s1, s2, w2 = k.measure()
+    c = k.counters()
+    assert c["removals"] == 0 and c["attempts"] == n * L * L
+    assert int(s1[0]) - L * L // 2 == 2 * c["deposits"]            # +2 per accepted flip, exactly
+    assert 0.25 < w2[0] < 1.0
+    _window_check(pkg, k, L, T, 1.0, 0.0, seed, n, L - 300, L - 300, 600, check_h00=True)   # wraps, holds (0,0)
+    _window_check(pkg, k, L, T, 1.0, 0.0, seed, n, 50000, 77777, 512)
+    _window_check(pkg, k, L, T, 1.0, 0.0, seed, n, L // 2 - 100, 3, 512)
+    k.close()
+    torch.cuda.empty_cache()
+
+
+def test_config5_shape_general_pq(pkg):
+    """BASELINE config 5 parameters (p=0.75, q=0.25, T=64, seed 3): full parity at L=8192, windows at L=2^19
+    when KPZ_TEST_2P19=1 (64 GiB of HBM)."""
+    import torch
+    L, T, seed = 8192, 64, 3
+    k = pkg.KPZ(L, 0.75, 0.25, T, seed)
+    k.init_flat()
+    o = Oracle(L, 0.75, 0.25, T, seed, threads=NTHREADS)
+    o.init_flat()
+    for t in range(3):
+        k.run(1); o.run(1)
+        _compare_scalars(k, [o])
+        assert k.state_hash() == o.state_hash()
+    _compare_full(k, o)
+    k.close()
+    if os.environ.get("KPZ_TEST_2P19", "0") == "1":
+        torch.cuda.empty_cache()
+        L, n = 1 << 19, 2
+        k = pkg.KPZ(L, 0.75, 0.25, T, seed)
+        k.init_flat(); k.run(n)
+        s1, s2, w2 = k.measure()
+        c = k.counters()
+        assert int(s1[0]) - L * L // 2 == 2 * (c["deposits"] - c["removals"])
+        _window_check(pkg, k, L, T, 0.75, 0.25, seed, n, L - 256, L - 256, 512, check_h00=True)
+        _window_check(pkg, k, L, T, 0.75, 0.25, seed, n, 400000, 123456, 512)
+        k.close()
+        torch.cuda.empty_cache()
