@@ -182,12 +182,120 @@ __device__ __forceinline__ void store_line(uint32_t* __restrict__ line, uint32_t
     }
 }
 
+// Stages / writes back one plane of a tile: lines line0 .. line0+T (periodic in L) of `plane`, T bits of each
+// starting at bit offset o.  Global accesses are issued KPZ-batch lines at a time, all loads of a batch before the
+// first dependent use, so that one thread keeps tens of requests in flight (one warp per CTA, ~6 warps per SM:
+// memory-level parallelism has to come from inside the thread).
+template <int T>
+struct StageBatch {
+    static constexpr int N = (T == 64) ? 13 : (T == 32) ? 11 : (T == 16) ? 17 : (T + 1);   // divides T+1
+};
+
+template <int T, int NTHR>
+__device__ __forceinline__ void load_plane(const uint32_t* __restrict__ plane, uint32_t L, uint32_t W, uint32_t line0,
+                                           uint32_t o, uint32_t* sm_plane) {
+    using G = TileGeom<T>;
+    constexpr int NB = StageBatch<T>::N;
+    const uint32_t s = o & 31u;
+    uint32_t idx[G::WPL + 1];
+    idx[0] = o >> 5;
+#pragma unroll
+    for (int k = 1; k <= G::WPL; ++k) idx[k] = (idx[k - 1] + 1u == W) ? 0u : idx[k - 1] + 1u;
+#pragma unroll 1
+    for (int l0 = 0; l0 <= T; l0 += NB) {
+        uint32_t raw[NB][G::WPL + 1];
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            uint32_t g = line0 + (uint32_t)(l0 + b);
+            if (g >= L) g -= L;
+            const uint32_t* line = plane + (size_t)g * W;
+#pragma unroll
+            for (int k = 0; k <= G::WPL; ++k) raw[b][k] = line[idx[k]];
+        }
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+#pragma unroll
+            for (int k = 0; k < G::WPL; ++k) {
+                uint32_t v = __funnelshift_r(raw[b][k], raw[b][k + 1], s);
+                if (T < 32) v &= G::LINE_MASK;
+                sm_plane[((l0 + b) * G::WPL + k) * NTHR] = v;
+            }
+        }
+    }
+}
+
+template <int T, int NTHR>
+__device__ __forceinline__ void store_plane(uint32_t* __restrict__ plane, uint32_t L, uint32_t W, uint32_t line0,
+                                            uint32_t o, const uint32_t* sm_plane) {
+    using G = TileGeom<T>;
+    if (T >= 32) {
+        constexpr int NB = StageBatch<T>::N;
+        const uint32_t s = o & 31u;
+        uint32_t idx[G::WPL + 1];
+        idx[0] = o >> 5;
+#pragma unroll
+        for (int k = 1; k <= G::WPL; ++k) idx[k] = (idx[k - 1] + 1u == W) ? 0u : idx[k - 1] + 1u;
+        if (s == 0u) {
+#pragma unroll 1
+            for (int l0 = 0; l0 <= T; l0 += NB) {
+#pragma unroll
+                for (int b = 0; b < NB; ++b) {
+                    uint32_t g = line0 + (uint32_t)(l0 + b);
+                    if (g >= L) g -= L;
+                    uint32_t* line = plane + (size_t)g * W;
+#pragma unroll
+                    for (int k = 0; k < G::WPL; ++k) line[idx[k]] = sm_plane[((l0 + b) * G::WPL + k) * NTHR];
+                }
+            }
+        } else {
+            // the first and last word of a line are shared with the (inactive) neighbour tiles: their bits are
+            // re-read and merged.  No other active tile touches these words.
+            const uint32_t lowmask = (1u << s) - 1u;
+#pragma unroll 1
+            for (int l0 = 0; l0 <= T; l0 += NB) {
+                uint32_t first[NB], last[NB];
+#pragma unroll
+                for (int b = 0; b < NB; ++b) {
+                    uint32_t g = line0 + (uint32_t)(l0 + b);
+                    if (g >= L) g -= L;
+                    const uint32_t* line = plane + (size_t)g * W;
+                    first[b] = line[idx[0]];
+                    last[b] = line[idx[G::WPL]];
+                }
+#pragma unroll
+                for (int b = 0; b < NB; ++b) {
+                    uint32_t g = line0 + (uint32_t)(l0 + b);
+                    if (g >= L) g -= L;
+                    uint32_t* line = plane + (size_t)g * W;
+                    uint32_t carry = first[b] & lowmask;
+#pragma unroll
+                    for (int k = 0; k < G::WPL; ++k) {
+                        const uint32_t v = sm_plane[((l0 + b) * G::WPL + k) * NTHR];
+                        line[idx[k]] = carry | (v << s);
+                        carry = v >> (32u - s);
+                    }
+                    line[idx[G::WPL]] = (last[b] & ~lowmask) | carry;
+                }
+            }
+        }
+    } else {
+#pragma unroll 4
+        for (int l = 0; l <= T; ++l) {
+            uint32_t g = line0 + (uint32_t)l;
+            if (g >= L) g -= L;
+            store_line<T, NTHR>(plane + (size_t)g * W, W, o, sm_plane + (l * G::WPL) * NTHR);
+        }
+    }
+}
+
 // One attempt (eq. 2).  MODE 0: p = 1, q = 0 (accept word never needed -- bit-identical, the generator is
 // counter-based).  MODE 1: general p, q.  TRACK: this thread's tile holds global site (0,0) at local index origin_idx.
+// A flip is four shared-memory XOR reductions (ATOMS.XOR without return): no ALU work for the new words, and
+// later loads of the same thread to the same address observe them (same-thread program order).
+// Deposits are not counted here: n_dep - n_rem is recovered from the first moment of the X lines (weight_x below).
 template <int T, int NTHR, int MODE, bool TRACK>
 __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site_word, uint32_t accept_word,
-                                        const UpdateParams& P, uint32_t& n_dep, uint32_t& n_rem, int32_t& dh00,
-                                        uint32_t origin_idx) {
+                                        const UpdateParams& P, uint32_t& n_rem, int32_t& dh00, uint32_t origin_idx) {
     using G = TileGeom<T>;
     const uint32_t idx = site_word >> (32 - 2 * G::LOG2T);      // mulhi32(site_word, T*T)
     const uint32_t lx = idx & (uint32_t)(T - 1);
@@ -203,36 +311,66 @@ __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site
     bool flip;
     if (MODE == 0) {
         flip = is_min;
-        n_dep += flip ? 1u : 0u;
         if (TRACK) dh00 += (flip && idx == origin_idx) ? 2 : 0;
     } else {
         const bool is_max = ((xa & ~xb & bx) != 0u) && ((ya & ~yb & by) != 0u);
         const bool dep = is_min && ((uint64_t)accept_word < P.thr_p);
         const bool rem = is_max && ((uint64_t)accept_word < P.thr_q);
         flip = dep || rem;
-        n_dep += dep ? 1u : 0u;
         n_rem += rem ? 1u : 0u;
         if (TRACK) dh00 += (idx == origin_idx) ? (dep ? 2 : (rem ? -2 : 0)) : 0;
     }
-    if (flip) {
-        px[0] = xa ^ bx;
-        px[G::WPL * NTHR] = xb ^ bx;
-        py[0] = ya ^ by;
-        py[G::WPL * NTHR] = yb ^ by;
+    // unconditional XOR reductions with a zero mask when nothing flips: no branch, so the whole batch stays one
+    // basic block for the instruction scheduler (ptxas branches around predicated ATOMS)
+    const uint32_t mx = flip ? bx : 0u, my = flip ? by : 0u;
+    atomicXor(px, mx);
+    atomicXor(px + G::WPL * NTHR, mx);
+    atomicXor(py, my);
+    atomicXor(py + G::WPL * NTHR, my);
+}
+
+// T*T sequential attempts of one tile.  Philox calls are generated KPZ_BATCH at a time, one batch ahead of the
+// attempts that consume them (the generator is counter-based, so the next batch does not depend on the lattice):
+// the integer pipes work on batch b+1 while the shared-memory round trips of batch b are in flight.
+template <int T, int NTHR, int MODE, bool TRACK>
+__device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const UpdateParams& P, uint32_t tile_id,
+                                               uint32_t replica, uint32_t& n_rem, int32_t& dh00,
+                                               uint32_t origin_idx) {
+    constexpr uint32_t CALLS = (uint32_t)(T * T) / 2u;
+    constexpr uint32_t B = (CALLS >= 4u) ? 4u : CALLS;
+    uint4 cur[B], nxt[B];
+#pragma unroll
+    for (uint32_t k = 0; k < B; ++k) cur[k] = philox4x32_10(k, tile_id, P.m, replica, P.key);
+#pragma unroll 1
+    for (uint32_t c = 0; c < CALLS; c += B) {
+        // batch b+1 (the last iteration generates one unused batch: CALLS/B + 1 batches for CALLS/B used)
+#pragma unroll
+        for (uint32_t k = 0; k < B; ++k) nxt[k] = philox4x32_10(c + B + k, tile_id, P.m, replica, P.key);
+#pragma unroll
+        for (uint32_t k = 0; k < B; ++k) {
+            attempt<T, NTHR, MODE, TRACK>(sm, cur[k].x, cur[k].y, P, n_rem, dh00, origin_idx);
+            attempt<T, NTHR, MODE, TRACK>(sm, cur[k].z, cur[k].w, P, n_rem, dh00, origin_idx);
+        }
+#pragma unroll
+        for (uint32_t k = 0; k < B; ++k) cur[k] = nxt[k];
     }
 }
 
-template <int T, int NTHR, int MODE, bool TRACK>
-__device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const UpdateParams& P, uint32_t tile_id,
-                                               uint32_t replica, uint32_t& n_dep, uint32_t& n_rem, int32_t& dh00,
-                                               uint32_t origin_idx) {
-    constexpr uint32_t CALLS = (uint32_t)(T * T) / 2u;
-#pragma unroll 2
-    for (uint32_t c = 0; c < CALLS; ++c) {
-        const uint4 Q = philox4x32_10(c, tile_id, P.m, replica, P.key);
-        attempt<T, NTHR, MODE, TRACK>(sm, Q.x, Q.y, P, n_dep, n_rem, dh00, origin_idx);
-        attempt<T, NTHR, MODE, TRACK>(sm, Q.z, Q.w, P, n_dep, n_rem, dh00, origin_idx);
+// first moment of the X lines of this thread's tile: sum over lines lx = 0..T of lx * popcount(line lx).
+// A deposition at (lx,ly) moves a set bit from line lx+1 to line lx (-1), a removal does the opposite (+1):
+// n_dep - n_rem = weight_before - weight_after.
+template <int T, int NTHR>
+__device__ __forceinline__ uint32_t weight_x(const uint32_t* __restrict__ sm) {
+    using G = TileGeom<T>;
+    uint32_t s = 0;
+#pragma unroll 5
+    for (int l = 1; l <= T; ++l) {
+        uint32_t c = 0;
+#pragma unroll
+        for (int k = 0; k < G::WPL; ++k) c += __popc(sm[(l * G::WPL + k) * NTHR]);
+        s += (uint32_t)l * c;
     }
+    return s;
 }
 
 template <int T, int NTHR, int MODE>
@@ -269,48 +407,30 @@ __global__ void __launch_bounds__(NTHR) kpz_update_kernel(const UpdateParams P) 
     const uint32_t offX = (Y0 >= L) ? Y0 - L : Y0;   // bit offset inside an X line (a column): y direction
     const uint32_t offY = (X0 >= L) ? X0 - L : X0;   // bit offset inside a Y line (a row): x direction
 
-    uint32_t n_dep = 0, n_rem = 0;
+    uint32_t n_dep = 0, n_rem = 0, w_before = 0;
     int32_t dh00 = 0;
     uint32_t origin_idx = 0xFFFFFFFFu;
     if (active) {
         // ---- a2: stage tile + halo ----
-#pragma unroll 4
-        for (int l = 0; l <= T; ++l) {
-            uint32_t gx = offY + (uint32_t)l;
-            if (gx >= L) gx -= L;
-            load_line<T, NTHR>(planeX + (size_t)gx * W, W, offX, sm + (l * G::WPL) * NTHR);
-        }
-#pragma unroll 4
-        for (int l = 0; l <= T; ++l) {
-            uint32_t gy = offX + (uint32_t)l;
-            if (gy >= L) gy -= L;
-            load_line<T, NTHR>(planeY + (size_t)gy * W, W, offY, sm + (G::PLANE + l * G::WPL) * NTHR);
-        }
+        load_plane<T, NTHR>(planeX, L, W, offY, offX, sm);
+        load_plane<T, NTHR>(planeY, L, W, offX, offY, sm + G::PLANE * NTHR);
         // does this tile hold global site (0,0)?  local coordinates of it: (L - offY) mod L, (L - offX) mod L
         const uint32_t lx0 = (offY == 0u) ? 0u : L - offY;
         const uint32_t ly0 = (offX == 0u) ? 0u : L - offX;
         if (lx0 < (uint32_t)T && ly0 < (uint32_t)T) origin_idx = ly0 * T + lx0;
+        w_before = weight_x<T, NTHR>(sm);
     }
     const bool any_origin = __any_sync(0xFFFFFFFFu, origin_idx != 0xFFFFFFFFu);
     if (active) {
         // ---- a3 + a4: T*T sequential attempts ----
         if (any_origin)
-            run_tile_steps<T, NTHR, MODE, true>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx);
+            run_tile_steps<T, NTHR, MODE, true>(sm, P, tile_id, replica, n_rem, dh00, origin_idx);
         else
-            run_tile_steps<T, NTHR, MODE, false>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx);
+            run_tile_steps<T, NTHR, MODE, false>(sm, P, tile_id, replica, n_rem, dh00, origin_idx);
+        n_dep = w_before - weight_x<T, NTHR>(sm) + n_rem;
         // ---- a5: write back ----
-#pragma unroll 4
-        for (int l = 0; l <= T; ++l) {
-            uint32_t gx = offY + (uint32_t)l;
-            if (gx >= L) gx -= L;
-            store_line<T, NTHR>(planeX + (size_t)gx * W, W, offX, sm + (l * G::WPL) * NTHR);
-        }
-#pragma unroll 4
-        for (int l = 0; l <= T; ++l) {
-            uint32_t gy = offX + (uint32_t)l;
-            if (gy >= L) gy -= L;
-            store_line<T, NTHR>(planeY + (size_t)gy * W, W, offY, sm + (G::PLANE + l * G::WPL) * NTHR);
-        }
+        store_plane<T, NTHR>(planeX, L, W, offY, offX, sm);
+        store_plane<T, NTHR>(planeY, L, W, offX, offY, sm + G::PLANE * NTHR);
     }
     // ---- a6: bookkeeping ----
     const uint32_t rep0 = __shfl_sync(0xFFFFFFFFu, replica, 0);
