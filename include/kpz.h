@@ -21,9 +21,8 @@
  *   - There is no CPU fallback: without a CUDA device every call that needs one returns KPZ_ECUDA.
  *
  * Device layout of the lattice buffer, per replica r at byte offset
- * r * L*L/4:  plane X = sigma_x as L bit-lines, one per COLUMN x (32-bit words, bit (y & 31) of word
- * x*(L/32) + (y >> 5)), followed by plane Y = sigma_y as L bit-lines, one per ROW y (bit (x & 31) of word
- * y*(L/32) + (x >> 5)).  Bit 1 <=> sigma = +1.
+ * r * L*L/4:  plane X = sigma_x followed by plane Y = sigma_y, each as L bit-lines, one per ROW y
+ * (32-bit words, sigma(x,y) = bit (x & 31) of word y*(L/32) + (x >> 5)).  Bit 1 <=> sigma = +1.
  */
 #ifndef KPZ_B200_H
 #define KPZ_B200_H

@@ -1,8 +1,8 @@
 // kpz_device.cuh -- device code of the B200-native octahedron-KPZ hot path (sm_100a).
 //
 // Kernels:
-//   kpz_update_kernel<T,...>   steps a2-a6 of SURVEY 8(a): tile + halo staged into shared memory as bit-lines,
-//                              T*T sequential Philox-driven attempts per tile (eq. 2), write-back.
+//   kpz_update_kernel<T,...>   steps a2-a6 of SURVEY 8(a): tile + halo staged into shared memory as one height bit
+//                              per site, T*T sequential Philox-driven attempts per tile (eq. 2), write-back.
 //   kpz_fill_flat_kernel       flat zig-zag start.
 //   kpz_row0_prefix_kernel,    height reconstruction (eq. 3) as a per-column chunk monoid and the exact
 //   kpz_column_chunk_kernel,   integer sums of h and h^2 (eq. 4).
@@ -94,247 +94,344 @@ __device__ __forceinline__ void global_draw(const UpdateParams& P, uint32_t repl
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// Update kernel.  One THREAD owns one tile; the tile lives in shared memory as bit-lines:
-//   plane X: line lx in [0,T] (a COLUMN of the tile; line T is the +x halo), bit ly  <=> sigma_x(X0+lx, Y0+ly)
-//   plane Y: line ly in [0,T] (a ROW of the tile;    line T is the +y halo), bit lx  <=> sigma_y(X0+lx, Y0+ly)
-// so that the pair (sigma_x(x,y), sigma_x(x+1,y)) is the same bit of two consecutive X lines and
-// (sigma_y(x,y), sigma_y(x,y+1)) the same bit of two consecutive Y lines: no straddling, no halo special case.
-// Word w of thread t sits at smem[w * NTHR + t]: every thread stays in its own bank -> conflict-free for any
-// access pattern.  Threads never share data: no barrier anywhere in the kernel.
+// Update kernel.  One THREAD owns one tile for all of its T*T sequential attempts (program order = schedule
+// order S3).  In shared memory the tile is NOT kept as slopes but as ONE bit per site, the high bit h1 of the
+// height modulo 4:
+//   in-tile heights are taken relative to an anchor of the right parity, h = 2*h1 + h0 (mod 4) with the low bit
+//   h0(lx,ly) = (lx+ly) & 1 fixed for ever (every step of the surface is +-1, every flip is +-2).  Then
+//     local minimum at a site with parity pi  <=>  all four neighbours have h1 == own_h1 ^ pi,
+//     local maximum                           <=>  all four neighbours have h1 != own_h1 ^ pi,
+//     a flip in either direction              <=>  XOR of the site's own h1 bit  (one shared-memory reduction).
+// Rows ly = -1 .. T (row index r = ly+1) hold the tile plus its 1-site halo on all four sides (the -x / -y
+// halos carry sigma_x(x0,.) / sigma_y(.,y0), which belong to the tile's own sites; the +x / +y halos are the slopes
+// on the inactive neighbours that a border update changes).
+//   T >= 32: a row is WPL = T/32 own words (bit lx&31 of word lx>>5) followed by one halo word H_r with
+//            bit 0 = h1(T, ly) and bit 31 = h1(-1, ly+1): the word before / after any own word then supplies the
+//            left / right neighbour of its bit 0 / bit 31 through one funnel shift -- no special case at the border.
+//   T <  32: a row is one word, bit p = lx+1 (bit 0 and bit T+1 are the halos).
+// Word w of thread t sits at smem[w * NTHR + t]: every thread stays in its own bank (conflict-free for any
+// access pattern) and threads never share data: no barrier anywhere in the kernel.
 // ------------------------------------------------------------------------------------------------------------
 template <int T>
 struct TileGeom {
     static constexpr int LOG2T = (T == 4) ? 2 : (T == 8) ? 3 : (T == 16) ? 4 : (T == 32) ? 5 : 6;
-    static constexpr int WPL = (T + 31) / 32;          // words per line
-    static constexpr int LINES = T + 1;
-    static constexpr int PLANE = LINES * WPL;
-    static constexpr int WORDS = 2 * PLANE;            // per tile
+    static constexpr bool WIDE = (T >= 32);
+    static constexpr int WPL = WIDE ? T / 32 : 1;      // own words per row
+    static constexpr int WPR = WIDE ? WPL + 1 : 1;     // words per row in shared memory
+    static constexpr int ROWS = T + 2;                 // ly = -1 .. T
+    static constexpr int PAD = WIDE ? 1 : 0;           // word "before" row 0 (never meaningful, keeps addresses valid)
+    static constexpr int WORDS = PAD + ROWS * WPR;     // per tile
     static constexpr uint32_t LINE_MASK = (T >= 32) ? 0xFFFFFFFFu : ((1u << (T & 31)) - 1u);
 };
 
-// loads T bits of a global bit-line starting at bit offset `o` (periodic in the line of W words)
-template <int T, int NTHR>
-__device__ __forceinline__ void load_line(const uint32_t* __restrict__ line, uint32_t W, uint32_t o, uint32_t* sm_line) {
-    using G = TileGeom<T>;
-    const uint32_t s = o & 31u;
-    uint32_t a = o >> 5;
-    uint32_t lo = __ldg(line + a);
-#pragma unroll
-    for (int k = 0; k < G::WPL; ++k) {
-        uint32_t a1 = a + 1u;
-        if (a1 == W) a1 = 0u;
-        const uint32_t hi = __ldg(line + a1);
-        uint32_t v = __funnelshift_r(lo, hi, s);
-        if (T < 32) v &= G::LINE_MASK;
-        sm_line[k * NTHR] = v;
-        lo = hi;
-        a = a1;
-    }
-}
-
-// stores T bits back (read-modify-write of the partially covered edge words / bytes; see DESIGN.md
-// "Halo write-back without races": no other active tile touches the same word (T >= 32) or byte (T < 32)).
-template <int T, int NTHR>
-__device__ __forceinline__ void store_line(uint32_t* __restrict__ line, uint32_t W, uint32_t o, const uint32_t* sm_line) {
-    using G = TileGeom<T>;
-    if (T >= 32) {
-        const uint32_t s = o & 31u;
-        uint32_t a = o >> 5;
-        if (s == 0u) {
-#pragma unroll
-            for (int k = 0; k < G::WPL; ++k) {
-                line[a] = sm_line[k * NTHR];
-                a = (a + 1u == W) ? 0u : a + 1u;
-            }
-        } else {
-            const uint32_t lowmask = (1u << s) - 1u;
-            uint32_t prev = line[a] & lowmask;     // bits below the segment stay
-            uint32_t carry = 0u;
-#pragma unroll
-            for (int k = 0; k < G::WPL; ++k) {
-                const uint32_t v = sm_line[k * NTHR];
-                const uint32_t out = (k == 0 ? prev : carry) | (v << s);
-                line[a] = out;
-                carry = v >> (32u - s);
-                a = (a + 1u == W) ? 0u : a + 1u;
-            }
-            line[a] = (line[a] & ~lowmask) | carry;
-        }
-    } else {
-        // byte granularity; o is a multiple of 4, T in {4, 8, 16}
-        uint8_t* bl = reinterpret_cast<uint8_t*>(line);
-        const uint32_t nbytes_line = W * 4u;
-        const uint32_t v = sm_line[0] & G::LINE_MASK;
-        const uint32_t sh = o & 7u;                          // 0 or 4
-        const uint32_t span = v << sh;                       // <= 20 bits
-        const uint32_t mask = G::LINE_MASK << sh;
-        uint32_t b = o >> 3;
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const uint32_t mk = (mask >> (8 * k)) & 0xFFu;
-            if (mk) {
-                const uint32_t nv = (span >> (8 * k)) & 0xFFu;
-                if (mk == 0xFFu) bl[b] = (uint8_t)nv;
-                else bl[b] = (uint8_t)((bl[b] & ~mk) | nv);
-            }
-            b = (b + 1u == nbytes_line) ? 0u : b + 1u;
-        }
-    }
-}
-
-// Stages / writes back one plane of a tile: lines line0 .. line0+T (periodic in L) of `plane`, T bits of each
-// starting at bit offset o.  Global accesses are issued KPZ-batch lines at a time, all loads of a batch before the
-// first dependent use, so that one thread keeps tens of requests in flight (one warp per CTA, ~6 warps per SM:
-// memory-level parallelism has to come from inside the thread).
+// rows fetched per batch while staging: all loads of a batch are issued before the first dependent use, so one
+// thread keeps tens of requests in flight.  N divides T+1.
 template <int T>
 struct StageBatch {
-    static constexpr int N = (T == 64) ? 13 : (T == 32) ? 11 : (T == 16) ? 17 : (T + 1);   // divides T+1
+    static constexpr int N = (T == 64) ? 13 : (T == 32) ? 11 : (T + 1);
 };
 
+// sigma_y(.,ly) = row(ly) ^ row(ly-1) ^ ycode(ly) and back (own columns, bit j <-> parity of lx):
+// h1(ly) = h1(ly-1) ^ XNOR(sigma_y(ly), h0(.,ly-1)),  h0(lx,ly-1) = (lx+ly-1)&1.
+__device__ __forceinline__ uint32_t ycode(uint32_t ly) { return 0xAAAAAAAAu ^ (0u - (ly & 1u)); }
+
+// inclusive prefix XOR over the 32 bits of a word
+__device__ __forceinline__ uint32_t prefix_xor32(uint32_t t) {
+    t ^= t << 1; t ^= t << 2; t ^= t << 4; t ^= t << 8; t ^= t << 16;
+    return t;
+}
+
+// ---- a2: stage tile + halo, slopes (HBM) -> height bits (shared memory), T >= 32 -----------------------------
 template <int T, int NTHR>
-__device__ __forceinline__ void load_plane(const uint32_t* __restrict__ plane, uint32_t L, uint32_t W, uint32_t line0,
-                                           uint32_t o, uint32_t* sm_plane) {
+__device__ __forceinline__ void stage_in_wide(const uint32_t* __restrict__ planeX, const uint32_t* __restrict__ planeY,
+                                              uint32_t L, uint32_t W, uint32_t x0, uint32_t y0, uint32_t* __restrict__ sm) {
     using G = TileGeom<T>;
     constexpr int NB = StageBatch<T>::N;
-    const uint32_t s = o & 31u;
-    uint32_t idx[G::WPL + 1];
-    idx[0] = o >> 5;
+    constexpr int WPL = G::WPL;
+    const uint32_t s = x0 & 31u;
+    uint32_t idx[WPL + 1];
+    idx[0] = x0 >> 5;
 #pragma unroll
-    for (int k = 1; k <= G::WPL; ++k) idx[k] = (idx[k - 1] + 1u == W) ? 0u : idx[k - 1] + 1u;
+    for (int k = 1; k <= WPL; ++k) idx[k] = (idx[k - 1] + 1u == W) ? 0u : idx[k - 1] + 1u;
+
+    // row ly = 0 from sigma_x(.,y0): h1(0,0) = 0 is the anchor, h1(lx,0) = XOR_{l=1..lx} XNOR(sigma_x(l), h0(l-1,0))
+    uint32_t prev[WPL];
+    {
+        const uint32_t* line = planeX + (size_t)y0 * W;
+        uint32_t raw[WPL + 1];
+#pragma unroll
+        for (int k = 0; k <= WPL; ++k) raw[k] = line[idx[k]];
+        uint32_t carry = 0u;
+#pragma unroll
+        for (int k = 0; k < WPL; ++k) {
+            uint32_t t = __funnelshift_r(raw[k], raw[k + 1], s) ^ 0xAAAAAAAAu;   // h0(l-1,0) = 1 for even l
+            if (k == 0) t &= ~1u;
+            t = prefix_xor32(t) ^ carry;
+            carry = 0u - (t >> 31);
+            prev[k] = t;
+        }
+    }
+    uint32_t pendingH = 0u;    // halo word of the previous row: bit 0 already holds its +x halo
 #pragma unroll 1
     for (int l0 = 0; l0 <= T; l0 += NB) {
-        uint32_t raw[NB][G::WPL + 1];
+        uint32_t ry[NB][WPL + 1], rx[NB][2];
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
-            uint32_t g = line0 + (uint32_t)(l0 + b);
+            uint32_t g = y0 + (uint32_t)(l0 + b);
             if (g >= L) g -= L;
-            const uint32_t* line = plane + (size_t)g * W;
+            const uint32_t* ly_ = planeY + (size_t)g * W;
+            const uint32_t* lx_ = planeX + (size_t)g * W;
 #pragma unroll
-            for (int k = 0; k <= G::WPL; ++k) raw[b][k] = line[idx[k]];
+            for (int k = 0; k <= WPL; ++k) ry[b][k] = ly_[idx[k]];
+            rx[b][0] = lx_[idx[0]];
+            rx[b][1] = lx_[idx[WPL]];
         }
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
+            const uint32_t ly = (uint32_t)(l0 + b);
+            const uint32_t r = ly + 1u;
+            uint32_t cur[WPL];
+            const uint32_t yc = ycode(ly);
+            if (b == 0 && l0 == 0) {
+                // rows -1 and 0:  row(-1) = row(0) ^ sigma_y(.,0) ^ ycode(0)
 #pragma unroll
-            for (int k = 0; k < G::WPL; ++k) {
-                uint32_t v = __funnelshift_r(raw[b][k], raw[b][k + 1], s);
-                if (T < 32) v &= G::LINE_MASK;
-                sm_plane[((l0 + b) * G::WPL + k) * NTHR] = v;
+                for (int k = 0; k < WPL; ++k) {
+                    const uint32_t yv = __funnelshift_r(ry[b][k], ry[b][k + 1], s);
+                    cur[k] = prev[k];
+                    sm[(G::PAD + k) * NTHR] = prev[k] ^ yv ^ yc;
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < WPL; ++k) {
+                    const uint32_t yv = __funnelshift_r(ry[b][k], ry[b][k + 1], s);
+                    cur[k] = prev[k] ^ yv ^ yc;
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < WPL; ++k) sm[(G::PAD + r * G::WPR + k) * NTHR] = cur[k];
+            if (ly < (uint32_t)T) {
+                // halos of this row from sigma_x(x0, y) and sigma_x(x0+T, y):  h1(A) = h1(B) ^ sigma ^ (ly & 1)
+                const uint32_t bL = (rx[b][0] >> s) & 1u, bR = (rx[b][1] >> s) & 1u;
+                const uint32_t hL = (cur[0] ^ bL ^ ly) & 1u;
+                const uint32_t hR = ((cur[WPL - 1] >> 31) ^ bR ^ ly) & 1u;
+                sm[(G::PAD + (r - 1u) * G::WPR + WPL) * NTHR] = pendingH | (hL << 31);
+                pendingH = hR;
+            } else {
+                sm[(G::PAD + (r - 1u) * G::WPR + WPL) * NTHR] = pendingH;
+            }
+#pragma unroll
+            for (int k = 0; k < WPL; ++k) prev[k] = cur[k];
+        }
+    }
+}
+
+// ---- a5: write back, height bits -> slopes, T >= 32.  The first and last word of a row segment are shared with
+// the (inactive, other-colour) neighbour tiles: re-read and merged.  No other thread of the launch touches
+// these words.
+template <int T, int NTHR>
+__device__ __forceinline__ void stage_out_wide(uint32_t* __restrict__ planeX, uint32_t* __restrict__ planeY, uint32_t L,
+                                               uint32_t W, uint32_t x0, uint32_t y0, const uint32_t* __restrict__ sm) {
+    using G = TileGeom<T>;
+    constexpr int NB = StageBatch<T>::N;
+    constexpr int WPL = G::WPL;
+    const uint32_t s = x0 & 31u;
+    const uint32_t lowmask = (1u << s) - 1u;            // bits below the segment start
+    const uint32_t lowmask1 = lowmask | (1u << s);      // ... and the bit that holds sigma_x(x0+T)
+    uint32_t idx[WPL + 1];
+    idx[0] = x0 >> 5;
+#pragma unroll
+    for (int k = 1; k <= WPL; ++k) idx[k] = (idx[k - 1] + 1u == W) ? 0u : idx[k - 1] + 1u;
+#pragma unroll 1
+    for (int l0 = 0; l0 <= T; l0 += NB) {
+        uint32_t ex[NB][2], ey[NB][2];
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            uint32_t g = y0 + (uint32_t)(l0 + b);
+            if (g >= L) g -= L;
+            const uint32_t* ly_ = planeY + (size_t)g * W;
+            const uint32_t* lx_ = planeX + (size_t)g * W;
+            ey[b][0] = ly_[idx[0]];
+            ey[b][1] = ly_[idx[WPL]];
+            ex[b][0] = lx_[idx[0]];
+            ex[b][1] = lx_[idx[WPL]];
+        }
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            const uint32_t ly = (uint32_t)(l0 + b);
+            const uint32_t r = ly + 1u;
+            uint32_t g = y0 + ly;
+            if (g >= L) g -= L;
+            uint32_t* ly_ = planeY + (size_t)g * W;
+            uint32_t* lx_ = planeX + (size_t)g * W;
+            uint32_t cur[WPL], below[WPL];
+#pragma unroll
+            for (int k = 0; k < WPL; ++k) {
+                cur[k] = sm[(G::PAD + r * G::WPR + k) * NTHR];
+                below[k] = sm[(G::PAD + (r - 1u) * G::WPR + k) * NTHR];
+            }
+            // sigma_y(.,ly): T bits at bit offset x0
+            {
+                const uint32_t yc = ycode(ly);
+                uint32_t v[WPL];
+#pragma unroll
+                for (int k = 0; k < WPL; ++k) v[k] = cur[k] ^ below[k] ^ yc;
+                ly_[idx[0]] = (ey[b][0] & lowmask) | (v[0] << s);
+#pragma unroll
+                for (int k = 1; k < WPL; ++k) ly_[idx[k]] = __funnelshift_l(v[k - 1], v[k], s);
+                if (s != 0u) ly_[idx[WPL]] = (ey[b][1] & ~lowmask) | __funnelshift_l(v[WPL - 1], 0u, s);
+            }
+            // sigma_x(.,ly): T+1 bits (lx = 0..T) at bit offset x0; rows 0..T-1 only
+            if (ly < (uint32_t)T) {
+                const uint32_t hprev = sm[(G::PAD + (r - 1u) * G::WPR + WPL) * NTHR];   // bit 31 = h1(-1, ly)
+                const uint32_t hcur = sm[(G::PAD + r * G::WPR + WPL) * NTHR];           // bit 0  = h1(T, ly)
+                const uint32_t xc = ycode(ly);      // bit j = (j + ly) & 1 = h0(lx, ly)
+                uint32_t v[WPL];
+#pragma unroll
+                for (int k = 0; k < WPL; ++k) {
+                    const uint32_t left = __funnelshift_l(k == 0 ? hprev : cur[k - 1], cur[k], 1);
+                    v[k] = cur[k] ^ left ^ xc;
+                }
+                const uint32_t bitT = (hcur ^ (cur[WPL - 1] >> 31) ^ ly) & 1u;          // (T + ly) & 1 = ly & 1
+                lx_[idx[0]] = (ex[b][0] & lowmask) | (v[0] << s);
+#pragma unroll
+                for (int k = 1; k < WPL; ++k) lx_[idx[k]] = __funnelshift_l(v[k - 1], v[k], s);
+                lx_[idx[WPL]] = (ex[b][1] & ~lowmask1) | __funnelshift_l(v[WPL - 1], 0u, s) | (bitT << s);
             }
         }
+    }
+}
+
+// ---- T < 32: a row is one word, bit p = lx+1.  nbits bits of a periodic bit-line starting at bit offset o
+// (a multiple of 4; the segment may span two words). -----------------------------------------------------------
+__device__ __forceinline__ uint32_t load_bits(const uint32_t* __restrict__ line, uint32_t W, uint32_t o, uint32_t mask) {
+    const uint32_t a = o >> 5;
+    const uint32_t a1 = (a + 1u == W) ? 0u : a + 1u;
+    return __funnelshift_r(line[a], line[a1], o) & mask;
+}
+
+// Writes the bits selected by `mask` (in segment coordinates) of `seg`.  Two same-colour tiles may share a
+// 32-bit word (and, for T = 4, a byte) when T < 32, so only the CHANGED bits are applied, with an XOR reduction:
+// every bit of a segment belongs to exactly one active tile, hence old ^ new on its own bits is exact.
+__device__ __forceinline__ void store_bits(uint32_t* __restrict__ line, uint32_t W, uint32_t o, uint32_t mask, uint32_t seg) {
+    const uint32_t a = o >> 5;
+    const uint32_t a1 = (a + 1u == W) ? 0u : a + 1u;
+    const uint32_t old = __funnelshift_r(line[a], line[a1], o) & mask;
+    const uint32_t d = old ^ (seg & mask);
+    const uint32_t s = o & 31u;
+    const uint32_t dlo = d << s;
+    const uint32_t dhi = __funnelshift_l(d, 0u, s);      // d >> (32 - s), 0 for s = 0
+    if (dlo) atomicXor(line + a, dlo);
+    if (dhi) atomicXor(line + a1, dhi);
+}
+
+template <int T, int NTHR>
+__device__ __forceinline__ void stage_in_narrow(const uint32_t* __restrict__ planeX, const uint32_t* __restrict__ planeY,
+                                                uint32_t L, uint32_t W, uint32_t x0, uint32_t y0, uint32_t* __restrict__ sm) {
+    constexpr uint32_t MT = (1u << T) - 1u;          // T bits
+    constexpr uint32_t MT1 = (2u << T) - 1u;         // T+1 bits
+    uint32_t prev = 0u;                               // h1 of the previous row, bit lx
+#pragma unroll 1
+    for (uint32_t ly = 0; ly <= (uint32_t)T; ++ly) {
+        uint32_t g = y0 + ly;
+        if (g >= L) g -= L;
+        const uint32_t yv = load_bits(planeY + (size_t)g * W, W, x0, MT);
+        const uint32_t xv = load_bits(planeX + (size_t)g * W, W, x0, MT1);
+        const uint32_t yc = ycode(ly) & MT;
+        uint32_t cur;
+        if (ly == 0u) {
+            cur = prefix_xor32((xv ^ 0xAAAAAAAAu) & MT & ~1u) & MT;
+            sm[0] = ((cur ^ yv ^ yc) & MT) << 1;                       // row -1: own columns only
+        } else {
+            cur = prev ^ yv ^ yc;
+        }
+        uint32_t word = cur << 1;
+        if (ly < (uint32_t)T) {
+            const uint32_t hL = (cur ^ xv ^ ly) & 1u;
+            const uint32_t hR = ((cur >> (T - 1)) ^ (xv >> T) ^ ly) & 1u;
+            word |= hL | (hR << (T + 1));
+        }
+        sm[(ly + 1u) * NTHR] = word;
+        prev = cur;
     }
 }
 
 template <int T, int NTHR>
-__device__ __forceinline__ void store_plane(uint32_t* __restrict__ plane, uint32_t L, uint32_t W, uint32_t line0,
-                                            uint32_t o, const uint32_t* sm_plane) {
-    using G = TileGeom<T>;
-    if (T >= 32) {
-        constexpr int NB = StageBatch<T>::N;
-        const uint32_t s = o & 31u;
-        uint32_t idx[G::WPL + 1];
-        idx[0] = o >> 5;
-#pragma unroll
-        for (int k = 1; k <= G::WPL; ++k) idx[k] = (idx[k - 1] + 1u == W) ? 0u : idx[k - 1] + 1u;
-        if (s == 0u) {
+__device__ __forceinline__ void stage_out_narrow(uint32_t* __restrict__ planeX, uint32_t* __restrict__ planeY, uint32_t L,
+                                                 uint32_t W, uint32_t x0, uint32_t y0, const uint32_t* __restrict__ sm) {
+    constexpr uint32_t MT = (1u << T) - 1u;
+    constexpr uint32_t MT1 = (2u << T) - 1u;
 #pragma unroll 1
-            for (int l0 = 0; l0 <= T; l0 += NB) {
-#pragma unroll
-                for (int b = 0; b < NB; ++b) {
-                    uint32_t g = line0 + (uint32_t)(l0 + b);
-                    if (g >= L) g -= L;
-                    uint32_t* line = plane + (size_t)g * W;
-#pragma unroll
-                    for (int k = 0; k < G::WPL; ++k) line[idx[k]] = sm_plane[((l0 + b) * G::WPL + k) * NTHR];
-                }
-            }
-        } else {
-            // the first and last word of a line are shared with the (inactive) neighbour tiles: their bits are
-            // re-read and merged.  No other active tile touches these words.
-            const uint32_t lowmask = (1u << s) - 1u;
-#pragma unroll 1
-            for (int l0 = 0; l0 <= T; l0 += NB) {
-                uint32_t first[NB], last[NB];
-#pragma unroll
-                for (int b = 0; b < NB; ++b) {
-                    uint32_t g = line0 + (uint32_t)(l0 + b);
-                    if (g >= L) g -= L;
-                    const uint32_t* line = plane + (size_t)g * W;
-                    first[b] = line[idx[0]];
-                    last[b] = line[idx[G::WPL]];
-                }
-#pragma unroll
-                for (int b = 0; b < NB; ++b) {
-                    uint32_t g = line0 + (uint32_t)(l0 + b);
-                    if (g >= L) g -= L;
-                    uint32_t* line = plane + (size_t)g * W;
-                    uint32_t carry = first[b] & lowmask;
-#pragma unroll
-                    for (int k = 0; k < G::WPL; ++k) {
-                        const uint32_t v = sm_plane[((l0 + b) * G::WPL + k) * NTHR];
-                        line[idx[k]] = carry | (v << s);
-                        carry = v >> (32u - s);
-                    }
-                    line[idx[G::WPL]] = (last[b] & ~lowmask) | carry;
-                }
-            }
-        }
-    } else {
-#pragma unroll 4
-        for (int l = 0; l <= T; ++l) {
-            uint32_t g = line0 + (uint32_t)l;
-            if (g >= L) g -= L;
-            store_line<T, NTHR>(plane + (size_t)g * W, W, o, sm_plane + (l * G::WPL) * NTHR);
+    for (uint32_t ly = 0; ly <= (uint32_t)T; ++ly) {
+        uint32_t g = y0 + ly;
+        if (g >= L) g -= L;
+        const uint32_t word = sm[(ly + 1u) * NTHR], below = sm[ly * NTHR];
+        const uint32_t sy = ((word ^ below) >> 1) ^ ycode(ly);
+        store_bits(planeY + (size_t)g * W, W, x0, MT, sy);
+        if (ly < (uint32_t)T) {
+            const uint32_t sx = ((word ^ (word << 1)) >> 1) ^ ycode(ly);   // bit lx = h1(lx)^h1(lx-1)^h0(lx,ly), lx = 0..T
+            store_bits(planeX + (size_t)g * W, W, x0, MT1, sx);
         }
     }
 }
 
-// One attempt (eq. 2).  MODE 0: p = 1, q = 0 (accept word never needed -- bit-identical, the generator is
-// counter-based).  MODE 1: general p, q.  TRACK: this thread's tile holds global site (0,0) at local index origin_idx.
-// A flip is four shared-memory XOR reductions (ATOMS.XOR without return): no ALU work for the new words, and
-// later loads of the same thread to the same address observe them (same-thread program order).
-// Deposits are not counted here: n_dep - n_rem is recovered from the first moment of the X lines (weight_x below).
+// ---- a4: one attempt (eq. 2).  MODE 0: p = 1, q = 0 (the accept word is never needed -- bit-identical, the
+// generator is counter-based).  MODE 1: general p, q.  TRACK: this thread's tile holds global site (0,0) at
+// local index origin_idx.  The flip is one shared-memory XOR reduction (ATOMS.XOR without return) with a zero
+// mask when nothing flips: no branch, so a whole batch of attempts stays one basic block for the scheduler.
 template <int T, int NTHR, int MODE, bool TRACK>
 __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site_word, uint32_t accept_word,
-                                        const UpdateParams& P, uint32_t& n_rem, int32_t& dh00, uint32_t origin_idx) {
+                                        const UpdateParams& P, uint32_t& n_dep, uint32_t& n_rem, int32_t& dh00,
+                                        uint32_t origin_idx) {
     using G = TileGeom<T>;
-    const uint32_t idx = site_word >> (32 - 2 * G::LOG2T);      // mulhi32(site_word, T*T)
-    const uint32_t lx = idx & (uint32_t)(T - 1);
+    const uint32_t idx = site_word >> (32 - 2 * G::LOG2T);      // mulhi32(site_word, T*T) = ly*T + lx
     const uint32_t ly = idx >> G::LOG2T;
-    uint32_t* px = sm + (lx * G::WPL + (T > 32 ? (ly >> 5) : 0u)) * NTHR;
-    uint32_t* py = sm + (G::PLANE + ly * G::WPL + (T > 32 ? (lx >> 5) : 0u)) * NTHR;
-    const uint32_t xa = px[0], xb = px[G::WPL * NTHR];
-    const uint32_t ya = py[0], yb = py[G::WPL * NTHR];
-    const uint32_t bx = 1u << (ly & 31u);
-    const uint32_t by = 1u << (lx & 31u);
-    // local minimum: sigma_x(x)=-1, sigma_x(x+1)=+1, sigma_y(y)=-1, sigma_y(y+1)=+1  (bits 0,1,0,1)
-    const bool is_min = ((~xa & xb & bx) != 0u) && ((~ya & yb & by) != 0u);
-    bool flip;
-    if (MODE == 0) {
-        flip = is_min;
-        if (TRACK) dh00 += (flip && idx == origin_idx) ? 2 : 0;
+    uint32_t* a;
+    uint32_t wo, wl, wr, sh, par;
+    if constexpr (G::WIDE) {
+        // word (row ly+1, k = lx>>5) = PAD + (ly+1)*WPR + k, and idx>>5 = ly*WPL + k
+        a = sm + ((idx >> 5) + ly + (uint32_t)(G::PAD + G::WPR)) * NTHR;
+        wo = a[0];
+        const uint32_t wp = *(a - NTHR), wn = a[NTHR];
+        wl = __funnelshift_l(wp, wo, 1);      // left neighbours aligned with their site
+        wr = __funnelshift_r(wo, wn, 1);      // right neighbours
+        sh = idx;                             // low 5 bits = lx & 31
+        par = ly;
     } else {
-        const bool is_max = ((xa & ~xb & bx) != 0u) && ((ya & ~yb & by) != 0u);
-        const bool dep = is_min && ((uint64_t)accept_word < P.thr_p);
-        const bool rem = is_max && ((uint64_t)accept_word < P.thr_q);
-        flip = dep || rem;
-        n_rem += rem ? 1u : 0u;
-        if (TRACK) dh00 += (idx == origin_idx) ? (dep ? 2 : (rem ? -2 : 0)) : 0;
+        a = sm + (ly + 1u) * NTHR;
+        wo = a[0];
+        wl = wo << 1;
+        wr = wo >> 1;
+        sh = (idx & (uint32_t)(T - 1)) + 1u;
+        par = ly + 1u;
     }
-    // unconditional XOR reductions with a zero mask when nothing flips: no branch, so the whole batch stays one
-    // basic block for the instruction scheduler (ptxas branches around predicated ATOMS)
-    const uint32_t mx = flip ? bx : 0u, my = flip ? by : 0u;
-    atomicXor(px, mx);
-    atomicXor(px + G::WPL * NTHR, mx);
-    atomicXor(py, my);
-    atomicXor(py + G::WPL * NTHR, my);
+    const uint32_t wd = *(a - G::WPR * NTHR), wu = a[G::WPR * NTHR];
+    // v: bit = own_h1 ^ pi at every position of the word (rotation of 0xAAAAAAAA by the row parity)
+    const uint32_t v = wo ^ __funnelshift_r(0xAAAAAAAAu, 0xAAAAAAAAu, par);
+    const uint32_t bit = __funnelshift_l(0u, 1u, sh);           // 1 << (sh & 31)
+    const uint32_t min_m = ~((wl ^ v) | (wr ^ v)) & ~((wd ^ v) | (wu ^ v)) & bit;
+    uint32_t m;
+    if (MODE == 0) {
+        m = min_m;
+        n_dep += __funnelshift_r(m, 0u, sh);
+        if (TRACK) dh00 += (m != 0u && idx == origin_idx) ? 2 : 0;
+    } else {
+        const uint32_t max_m = ((wl ^ v) & (wr ^ v)) & ((wd ^ v) & (wu ^ v)) & bit;
+        const uint32_t md = ((uint64_t)accept_word < P.thr_p) ? min_m : 0u;
+        const uint32_t mr = ((uint64_t)accept_word < P.thr_q) ? max_m : 0u;
+        m = md | mr;
+        n_dep += __funnelshift_r(md, 0u, sh);
+        n_rem += __funnelshift_r(mr, 0u, sh);
+        if (TRACK) dh00 += (idx == origin_idx) ? (md ? 2 : (mr ? -2 : 0)) : 0;
+    }
+    atomicXor(a, m);
 }
 
-// T*T sequential attempts of one tile.  Philox calls are generated KPZ_BATCH at a time, one batch ahead of the
-// attempts that consume them (the generator is counter-based, so the next batch does not depend on the lattice):
-// the integer pipes work on batch b+1 while the shared-memory round trips of batch b are in flight.
+// T*T sequential attempts of one tile.  Philox calls are generated B at a time, one batch ahead of the attempts
+// that consume them (the generator is counter-based, so the next batch does not depend on the lattice): the
+// integer pipes work on batch b+1 while the shared-memory round trips of batch b are in flight.
 template <int T, int NTHR, int MODE, bool TRACK>
 __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const UpdateParams& P, uint32_t tile_id,
-                                               uint32_t replica, uint32_t& n_rem, int32_t& dh00,
+                                               uint32_t replica, uint32_t& n_dep, uint32_t& n_rem, int32_t& dh00,
                                                uint32_t origin_idx) {
     constexpr uint32_t CALLS = (uint32_t)(T * T) / 2u;
     constexpr uint32_t B = (CALLS >= 4u) ? 4u : CALLS;
@@ -348,29 +445,12 @@ __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const 
         for (uint32_t k = 0; k < B; ++k) nxt[k] = philox4x32_10(c + B + k, tile_id, P.m, replica, P.key);
 #pragma unroll
         for (uint32_t k = 0; k < B; ++k) {
-            attempt<T, NTHR, MODE, TRACK>(sm, cur[k].x, cur[k].y, P, n_rem, dh00, origin_idx);
-            attempt<T, NTHR, MODE, TRACK>(sm, cur[k].z, cur[k].w, P, n_rem, dh00, origin_idx);
+            attempt<T, NTHR, MODE, TRACK>(sm, cur[k].x, cur[k].y, P, n_dep, n_rem, dh00, origin_idx);
+            attempt<T, NTHR, MODE, TRACK>(sm, cur[k].z, cur[k].w, P, n_dep, n_rem, dh00, origin_idx);
         }
 #pragma unroll
         for (uint32_t k = 0; k < B; ++k) cur[k] = nxt[k];
     }
-}
-
-// first moment of the X lines of this thread's tile: sum over lines lx = 0..T of lx * popcount(line lx).
-// A deposition at (lx,ly) moves a set bit from line lx+1 to line lx (-1), a removal does the opposite (+1):
-// n_dep - n_rem = weight_before - weight_after.
-template <int T, int NTHR>
-__device__ __forceinline__ uint32_t weight_x(const uint32_t* __restrict__ sm) {
-    using G = TileGeom<T>;
-    uint32_t s = 0;
-#pragma unroll 5
-    for (int l = 1; l <= T; ++l) {
-        uint32_t c = 0;
-#pragma unroll
-        for (int k = 0; k < G::WPL; ++k) c += __popc(sm[(l * G::WPL + k) * NTHR]);
-        s += (uint32_t)l * c;
-    }
-    return s;
 }
 
 template <int T, int NTHR, int MODE>
@@ -404,33 +484,31 @@ __global__ void __launch_bounds__(NTHR) kpz_update_kernel(const UpdateParams P) 
     uint32_t* planeX = P.lattice + (size_t)replica * 2u * P.plane_words;
     uint32_t* planeY = planeX + P.plane_words;
     const uint32_t L = P.L, W = P.W;
-    const uint32_t offX = (Y0 >= L) ? Y0 - L : Y0;   // bit offset inside an X line (a column): y direction
-    const uint32_t offY = (X0 >= L) ? X0 - L : X0;   // bit offset inside a Y line (a row): x direction
+    const uint32_t x0 = (X0 >= L) ? X0 - L : X0;   // first own column = bit offset inside a row
+    const uint32_t y0 = (Y0 >= L) ? Y0 - L : Y0;   // first own row
 
-    uint32_t n_dep = 0, n_rem = 0, w_before = 0;
+    uint32_t n_dep = 0, n_rem = 0;
     int32_t dh00 = 0;
     uint32_t origin_idx = 0xFFFFFFFFu;
     if (active) {
         // ---- a2: stage tile + halo ----
-        load_plane<T, NTHR>(planeX, L, W, offY, offX, sm);
-        load_plane<T, NTHR>(planeY, L, W, offX, offY, sm + G::PLANE * NTHR);
-        // does this tile hold global site (0,0)?  local coordinates of it: (L - offY) mod L, (L - offX) mod L
-        const uint32_t lx0 = (offY == 0u) ? 0u : L - offY;
-        const uint32_t ly0 = (offX == 0u) ? 0u : L - offX;
+        if constexpr (G::WIDE) stage_in_wide<T, NTHR>(planeX, planeY, L, W, x0, y0, sm);
+        else stage_in_narrow<T, NTHR>(planeX, planeY, L, W, x0, y0, sm);
+        // does this tile hold global site (0,0)?  its local coordinates: (L - x0) mod L, (L - y0) mod L
+        const uint32_t lx0 = (x0 == 0u) ? 0u : L - x0;
+        const uint32_t ly0 = (y0 == 0u) ? 0u : L - y0;
         if (lx0 < (uint32_t)T && ly0 < (uint32_t)T) origin_idx = ly0 * T + lx0;
-        w_before = weight_x<T, NTHR>(sm);
     }
     const bool any_origin = __any_sync(0xFFFFFFFFu, origin_idx != 0xFFFFFFFFu);
     if (active) {
         // ---- a3 + a4: T*T sequential attempts ----
         if (any_origin)
-            run_tile_steps<T, NTHR, MODE, true>(sm, P, tile_id, replica, n_rem, dh00, origin_idx);
+            run_tile_steps<T, NTHR, MODE, true>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx);
         else
-            run_tile_steps<T, NTHR, MODE, false>(sm, P, tile_id, replica, n_rem, dh00, origin_idx);
-        n_dep = w_before - weight_x<T, NTHR>(sm) + n_rem;
+            run_tile_steps<T, NTHR, MODE, false>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx);
         // ---- a5: write back ----
-        store_plane<T, NTHR>(planeX, L, W, offY, offX, sm);
-        store_plane<T, NTHR>(planeY, L, W, offX, offY, sm + G::PLANE * NTHR);
+        if constexpr (G::WIDE) stage_out_wide<T, NTHR>(planeX, planeY, L, W, x0, y0, sm);
+        else stage_out_narrow<T, NTHR>(planeX, planeY, L, W, x0, y0, sm);
     }
     // ---- a6: bookkeeping ----
     const uint32_t rep0 = __shfl_sync(0xFFFFFFFFu, replica, 0);
@@ -489,7 +567,7 @@ __global__ void kpz_row0_prefix_kernel(const uint32_t* __restrict__ lattice, uin
     const uint32_t x0 = threadIdx.x * seg;
     int32_t s = 0;
     for (uint32_t x = x0; x < x0 + seg && x < L; ++x) {
-        if (x > 0u) s += (int32_t)((planeX[(size_t)x * W] & 1u) << 1) - 1;    // sigma_x(x, 0)
+        if (x > 0u) s += (int32_t)(((planeX[x >> 5] >> (x & 31u)) & 1u) << 1) - 1;    // sigma_x(x, 0)
     }
     part[threadIdx.x] = s;
     __syncthreads();
@@ -503,7 +581,7 @@ __global__ void kpz_row0_prefix_kernel(const uint32_t* __restrict__ lattice, uin
     int32_t run = part[threadIdx.x] - s;      // sum over x < x0
     int32_t* out = base + (size_t)replica * L;
     for (uint32_t x = x0; x < x0 + seg && x < L; ++x) {
-        if (x > 0u) run += (int32_t)((planeX[(size_t)x * W] & 1u) << 1) - 1;
+        if (x > 0u) run += (int32_t)(((planeX[x >> 5] >> (x & 31u)) & 1u) << 1) - 1;
         out[x] = run;                         // h(x,0) - h(0,0)
     }
 }
@@ -602,7 +680,7 @@ __global__ void kpz_unpack_window_kernel(const uint32_t* __restrict__ lattice, u
     for (uint64_t t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += stride) {
         const uint32_t jj = (uint32_t)(t / w), ii = (uint32_t)(t - (uint64_t)jj * w);
         const uint32_t x = (x0 + ii) % L, y = (y0 + jj) % L;
-        const uint32_t bxv = (planeX[(size_t)x * W + (y >> 5)] >> (y & 31u)) & 1u;
+        const uint32_t bxv = (planeX[(size_t)y * W + (x >> 5)] >> (x & 31u)) & 1u;
         const uint32_t byv = (planeY[(size_t)y * W + (x >> 5)] >> (x & 31u)) & 1u;
         sx[t] = bxv ? 1 : -1;
         sy[t] = byv ? 1 : -1;
@@ -647,8 +725,8 @@ __global__ void kpz_pack_kernel(uint32_t* __restrict__ lattice, uint64_t plane_w
         uint32_t wx = 0, wy = 0;
         for (uint32_t b = 0; b < 32u; ++b) {
             const uint32_t c = 32u * k + b;
-            // plane X: line = x, c = y ; plane Y: line = y, c = x
-            if (sx[(size_t)c * L + line] > 0) wx |= 1u << b;
+            // both planes: line = y, c = x
+            if (sx[(size_t)line * L + c] > 0) wx |= 1u << b;
             if (sy[(size_t)line * L + c] > 0) wy |= 1u << b;
         }
         planeX[t] = wx;
@@ -673,11 +751,11 @@ __global__ void kpz_hash_kernel(const uint32_t* __restrict__ lattice, uint64_t p
     for (uint64_t t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; t < plane_words; t += stride) {
         const uint32_t line = (uint32_t)(t / W), k = (uint32_t)(t - (uint64_t)line * W);
         const uint32_t wy = planeY[t];      // row y = line, x = 32k + b
-        const uint32_t wx = planeX[t];      // column x = line, y = 32k + b
+        const uint32_t wx = planeX[t];      // same row, same columns
         for (uint32_t b = 0; b < 32u; ++b) {
             const uint32_t c = 32u * k + b;
             if ((wy >> b) & 1u) acc += mix64(2ull * ((uint64_t)line * L + c) + 1ull);
-            if ((wx >> b) & 1u) acc += mix64(2ull * ((uint64_t)c * L + line));
+            if ((wx >> b) & 1u) acc += mix64(2ull * ((uint64_t)line * L + c));
         }
     }
 #pragma unroll
