@@ -101,16 +101,15 @@ class Twin:
                 for ty in range(colour >> 1, NT, 2):
                     for tx in range(colour & 1, NT, 2):
                         tile_id = ty * NT + tx
-                        for call in range((T * T + 1) // 2):
-                            Q = philox4x32_10((call, tile_id, m, self.replica), self.key)
-                            for half in (0, 1):
-                                s = 2 * call + half
-                                if s >= T * T:
-                                    break
-                                idx = mulhi32(Q[2 * half], T * T)
-                                x = (ox + tx * T + idx % T) % L
-                                y = (oy + ty * T + idx // T) % L
-                                self._attempt(x, y, Q[2 * half + 1])
+                        for s in range(T * T):
+                            # steps 4b..4b+3: site words = call b, accept words = call b + 2^31 (S3)
+                            if s % 4 == 0:
+                                sites = philox4x32_10((s // 4, tile_id, m, self.replica), self.key)
+                                accepts = philox4x32_10((s // 4 + 0x80000000, tile_id, m, self.replica), self.key)
+                            idx = mulhi32(sites[s % 4], T * T)
+                            x = (ox + tx * T + idx % T) % L
+                            y = (oy + ty * T + idx // T) % L
+                            self._attempt(x, y, accepts[s % 4])
             self.mcs += 1
 
     def slopes(self):

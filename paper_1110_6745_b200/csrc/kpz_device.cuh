@@ -142,11 +142,10 @@ __device__ __forceinline__ uint32_t prefix_xor32(uint32_t t) {
 }
 
 // ---- a2: stage tile + halo, slopes (HBM) -> height bits (shared memory), T >= 32 -----------------------------
-template <int T, int NTHR>
+template <int T, int NTHR, int NB = StageBatch<T>::N>
 __device__ __forceinline__ void stage_in_wide(const uint32_t* __restrict__ planeX, const uint32_t* __restrict__ planeY,
                                               uint32_t L, uint32_t W, uint32_t x0, uint32_t y0, uint32_t* __restrict__ sm) {
     using G = TileGeom<T>;
-    constexpr int NB = StageBatch<T>::N;
     constexpr int WPL = G::WPL;
     const uint32_t s = x0 & 31u;
     uint32_t idx[WPL + 1];
@@ -228,11 +227,10 @@ __device__ __forceinline__ void stage_in_wide(const uint32_t* __restrict__ plane
 // ---- a5: write back, height bits -> slopes, T >= 32.  The first and last word of a row segment are shared with
 // the (inactive, other-colour) neighbour tiles: re-read and merged.  No other thread of the launch touches
 // these words.
-template <int T, int NTHR>
+template <int T, int NTHR, int NB = StageBatch<T>::N>
 __device__ __forceinline__ void stage_out_wide(uint32_t* __restrict__ planeX, uint32_t* __restrict__ planeY, uint32_t L,
                                                uint32_t W, uint32_t x0, uint32_t y0, const uint32_t* __restrict__ sm) {
     using G = TileGeom<T>;
-    constexpr int NB = StageBatch<T>::N;
     constexpr int WPL = G::WPL;
     const uint32_t s = x0 & 31u;
     const uint32_t lowmask = (1u << s) - 1u;            // bits below the segment start
@@ -374,10 +372,27 @@ __device__ __forceinline__ void stage_out_narrow(uint32_t* __restrict__ planeX, 
     }
 }
 
-// ---- a4: one attempt (eq. 2).  MODE 0: p = 1, q = 0 (the accept word is never needed -- bit-identical, the
-// generator is counter-based).  MODE 1: general p, q.  TRACK: this thread's tile holds global site (0,0) at
-// local index origin_idx.  The flip is one shared-memory XOR reduction (ATOMS.XOR without return) with a zero
-// mask when nothing flips: no branch, so a whole batch of attempts stays one basic block for the scheduler.
+// ---- a4: one attempt (eq. 2).  MODE 0: p = 1, q = 0 (accept words are never needed and their Philox calls are
+// never evaluated -- bit-identical, the generator is counter-based).  MODE 1: general p, q.  TRACK: this
+// thread's tile holds global site (0,0) at local index origin_idx.  A flip is one shared-memory XOR reduction
+// (ATOMS.XOR without return) with a zero mask when nothing flips: no branch on the outcome, so a whole batch of
+// attempts stays one basic block for the instruction scheduler.
+__device__ __forceinline__ uint32_t lop3_any_differs(uint32_t v, uint32_t a, uint32_t b) {
+    uint32_t r;   // (v ^ a) | (v ^ b)
+    asm("lop3.b32 %0, %1, %2, %3, 0x7e;" : "=r"(r) : "r"(v), "r"(a), "r"(b));
+    return r;
+}
+__device__ __forceinline__ uint32_t lop3_all_differ(uint32_t v, uint32_t a, uint32_t b) {
+    uint32_t r;   // (v ^ a) & (v ^ b)
+    asm("lop3.b32 %0, %1, %2, %3, 0x18;" : "=r"(r) : "r"(v), "r"(a), "r"(b));
+    return r;
+}
+__device__ __forceinline__ uint32_t lop3_and_not_not(uint32_t m, uint32_t x, uint32_t y) {
+    uint32_t r;   // m & ~x & ~y
+    asm("lop3.b32 %0, %1, %2, %3, 0x10;" : "=r"(r) : "r"(m), "r"(x), "r"(y));
+    return r;
+}
+
 template <int T, int NTHR, int MODE, bool TRACK>
 __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site_word, uint32_t accept_word,
                                         const UpdateParams& P, uint32_t& n_dep, uint32_t& n_rem, int32_t& dh00,
@@ -408,48 +423,65 @@ __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site
     // v: bit = own_h1 ^ pi at every position of the word (rotation of 0xAAAAAAAA by the row parity)
     const uint32_t v = wo ^ __funnelshift_r(0xAAAAAAAAu, 0xAAAAAAAAu, par);
     const uint32_t bit = __funnelshift_l(0u, 1u, sh);           // 1 << (sh & 31)
-    const uint32_t min_m = ~((wl ^ v) | (wr ^ v)) & ~((wd ^ v) | (wu ^ v)) & bit;
-    uint32_t m;
+    // local minimum <=> no neighbour differs from v
+    const uint32_t md0 = lop3_and_not_not(bit, lop3_any_differs(v, wl, wr), lop3_any_differs(v, wd, wu));
     if (MODE == 0) {
-        m = min_m;
-        n_dep += __funnelshift_r(m, 0u, sh);
-        if (TRACK) dh00 += (m != 0u && idx == origin_idx) ? 2 : 0;
+        atomicXor(a, md0);
+        n_dep += (md0 != 0u) ? 1u : 0u;
+        if (TRACK) dh00 += (md0 != 0u && idx == origin_idx) ? 2 : 0;
     } else {
-        const uint32_t max_m = ((wl ^ v) & (wr ^ v)) & ((wd ^ v) & (wu ^ v)) & bit;
-        const uint32_t md = ((uint64_t)accept_word < P.thr_p) ? min_m : 0u;
-        const uint32_t mr = ((uint64_t)accept_word < P.thr_q) ? max_m : 0u;
-        m = md | mr;
-        n_dep += __funnelshift_r(md, 0u, sh);
-        n_rem += __funnelshift_r(mr, 0u, sh);
+        // local maximum <=> every neighbour differs from v
+        const uint32_t mr0 = bit & lop3_all_differ(v, wl, wr) & lop3_all_differ(v, wd, wu);
+        const uint32_t md = ((uint64_t)accept_word < P.thr_p) ? md0 : 0u;
+        const uint32_t mr = ((uint64_t)accept_word < P.thr_q) ? mr0 : 0u;
+        atomicXor(a, md | mr);
+        n_dep += (md != 0u) ? 1u : 0u;
+        n_rem += (mr != 0u) ? 1u : 0u;
         if (TRACK) dh00 += (idx == origin_idx) ? (md ? 2 : (mr ? -2 : 0)) : 0;
     }
-    atomicXor(a, m);
 }
 
-// T*T sequential attempts of one tile.  Philox calls are generated B at a time, one batch ahead of the attempts
-// that consume them (the generator is counter-based, so the next batch does not depend on the lattice): the
-// integer pipes work on batch b+1 while the shared-memory round trips of batch b are in flight.
+// T*T sequential attempts of one tile (S3: steps 4c..4c+3 take their site words from call c and their accept
+// words from call c | 2^31).  Calls are generated B at a time, one batch ahead of the attempts that consume them
+// (the generator is counter-based, so the next batch does not depend on the lattice): the multiplier pipe works
+// on batch b+1 while the shared-memory round trips of batch b are in flight.
+#ifndef KPZ_PHILOX_BATCH
+#define KPZ_PHILOX_BATCH 2u
+#endif
 template <int T, int NTHR, int MODE, bool TRACK>
 __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const UpdateParams& P, uint32_t tile_id,
                                                uint32_t replica, uint32_t& n_dep, uint32_t& n_rem, int32_t& dh00,
                                                uint32_t origin_idx) {
-    constexpr uint32_t CALLS = (uint32_t)(T * T) / 2u;
-    constexpr uint32_t B = (CALLS >= 4u) ? 4u : CALLS;
-    uint4 cur[B], nxt[B];
+    constexpr uint32_t CALLS = (uint32_t)(T * T) / 4u;
+    constexpr uint32_t B = (CALLS >= KPZ_PHILOX_BATCH) ? KPZ_PHILOX_BATCH : CALLS;
+    constexpr uint32_t ACCEPT = 0x80000000u;
+    uint4 cur[B], nxt[B], cur_a[MODE ? B : 1u], nxt_a[MODE ? B : 1u];
 #pragma unroll
-    for (uint32_t k = 0; k < B; ++k) cur[k] = philox4x32_10(k, tile_id, P.m, replica, P.key);
+    for (uint32_t k = 0; k < B; ++k) {
+        cur[k] = philox4x32_10(k, tile_id, P.m, replica, P.key);
+        if (MODE) cur_a[k] = philox4x32_10(k | ACCEPT, tile_id, P.m, replica, P.key);
+    }
 #pragma unroll 1
     for (uint32_t c = 0; c < CALLS; c += B) {
         // batch b+1 (the last iteration generates one unused batch: CALLS/B + 1 batches for CALLS/B used)
 #pragma unroll
-        for (uint32_t k = 0; k < B; ++k) nxt[k] = philox4x32_10(c + B + k, tile_id, P.m, replica, P.key);
-#pragma unroll
         for (uint32_t k = 0; k < B; ++k) {
-            attempt<T, NTHR, MODE, TRACK>(sm, cur[k].x, cur[k].y, P, n_dep, n_rem, dh00, origin_idx);
-            attempt<T, NTHR, MODE, TRACK>(sm, cur[k].z, cur[k].w, P, n_dep, n_rem, dh00, origin_idx);
+            nxt[k] = philox4x32_10(c + B + k, tile_id, P.m, replica, P.key);
+            if (MODE) nxt_a[k] = philox4x32_10((c + B + k) | ACCEPT, tile_id, P.m, replica, P.key);
         }
 #pragma unroll
-        for (uint32_t k = 0; k < B; ++k) cur[k] = nxt[k];
+        for (uint32_t k = 0; k < B; ++k) {
+            const uint4 qa = MODE ? cur_a[k] : make_uint4(0u, 0u, 0u, 0u);
+            attempt<T, NTHR, MODE, TRACK>(sm, cur[k].x, qa.x, P, n_dep, n_rem, dh00, origin_idx);
+            attempt<T, NTHR, MODE, TRACK>(sm, cur[k].y, qa.y, P, n_dep, n_rem, dh00, origin_idx);
+            attempt<T, NTHR, MODE, TRACK>(sm, cur[k].z, qa.z, P, n_dep, n_rem, dh00, origin_idx);
+            attempt<T, NTHR, MODE, TRACK>(sm, cur[k].w, qa.w, P, n_dep, n_rem, dh00, origin_idx);
+        }
+#pragma unroll
+        for (uint32_t k = 0; k < B; ++k) {
+            cur[k] = nxt[k];
+            if (MODE) cur_a[k] = nxt_a[k];
+        }
     }
 }
 
@@ -535,6 +567,7 @@ __global__ void __launch_bounds__(NTHR) kpz_update_kernel(const UpdateParams P) 
         if (dh00) atomicAdd(st + 2, (unsigned long long)(long long)dh00);
     }
 }
+
 
 // ------------------------------------------------------------------------------------------------------------
 // Flat start: sigma_x = sigma_y = +1 iff (x+y) odd.  One thread per 32-bit word of a replica's two planes.
