@@ -144,17 +144,22 @@ void run_tile(Oracle* o, uint32_t m, uint32_t ox, uint32_t oy, uint32_t tx, uint
     const uint32_t tile_id = ty * o->NT + tx;
     const uint32_t key[2] = {(uint32_t)(o->seed & 0xFFFFFFFFu), (uint32_t)(o->seed >> 32)};
     const uint32_t steps = T * T;
-    // S3: steps 4b..4b+3 take their site words from call R(b, ...) and their accept words from call
-    // R(b | 0x80000000, ...), word s & 3 of each.
+    // S3: a 32-bit site word W is read as a base-T*T fraction and gives two site indices,
+    //   digit 0 = mulhi32(W, T*T),  digit 1 = mulhi32((W * T*T) mod 2^32, T*T);
+    // step s takes digit s & 1 of word (s >> 1) & 3 of call R(s >> 3, ...); its accept word is word s & 3 of call
+    // R((s >> 2) | 0x80000000, ...).
     uint32_t QS[4] = {0, 0, 0, 0}, QA[4] = {0, 0, 0, 0};
     for (uint32_t s = 0; s < steps; ++s) {
-        if ((s & 3u) == 0u) {
-            uint32_t ctr_s[4] = {s >> 2, tile_id, m, o->replica};
-            uint32_t ctr_a[4] = {(s >> 2) | 0x80000000u, tile_id, m, o->replica};
+        if ((s & 7u) == 0u) {
+            uint32_t ctr_s[4] = {s >> 3, tile_id, m, o->replica};
             philox4x32_10(ctr_s, key, QS);
+        }
+        if ((s & 3u) == 0u) {
+            uint32_t ctr_a[4] = {(s >> 2) | 0x80000000u, tile_id, m, o->replica};
             philox4x32_10(ctr_a, key, QA);
         }
-        uint32_t site_word = QS[s & 3u];
+        uint32_t site_word = QS[(s >> 1) & 3u];
+        if (s & 1u) site_word = site_word * steps;      // second digit: fractional part of W * T*T
         uint32_t accept_word = QA[s & 3u];
         uint32_t idx = mulhi32(site_word, steps);
         uint32_t lx = idx % T, ly = idx / T;
@@ -329,15 +334,15 @@ int kpzo_run_checked(void* h, uint64_t n_mcs) {
             uint32_t cx = perm[i] & 1u, cy = perm[i] >> 1;
             for (uint32_t ty = cy; ty < o->NT; ty += 2)
                 for (uint32_t tx = cx; tx < o->NT; tx += 2) {
-                    uint32_t QS[4] = {0, 0, 0, 0}, QA[4] = {0, 0, 0, 0};
                     for (uint32_t s = 0; s < T * T; ++s) {
-                        if ((s & 3u) == 0u) {
-                            uint32_t ctr_s[4] = {s >> 2, ty * o->NT + tx, m, o->replica};
-                            uint32_t ctr_a[4] = {(s >> 2) | 0x80000000u, ty * o->NT + tx, m, o->replica};
-                            philox4x32_10(ctr_s, key, QS);
-                            philox4x32_10(ctr_a, key, QA);
-                        }
-                        uint32_t idx = mulhi32(QS[s & 3u], T * T);
+                        uint32_t QS[4], QA[4];
+                        uint32_t ctr_s[4] = {s >> 3, ty * o->NT + tx, m, o->replica};
+                        uint32_t ctr_a[4] = {(s >> 2) | 0x80000000u, ty * o->NT + tx, m, o->replica};
+                        philox4x32_10(ctr_s, key, QS);
+                        philox4x32_10(ctr_a, key, QA);
+                        uint32_t site_word = QS[(s >> 1) & 3u];
+                        if (s & 1u) site_word = site_word * (T * T);
+                        uint32_t idx = mulhi32(site_word, T * T);
                         uint32_t x = (ox + tx * T + idx % T) % L, y = (oy + ty * T + idx / T) % L;
                         int64_t before = 0; for (size_t k = 0; k < (size_t)L * L; ++k) before += o->H[k];
                         int dir = attempt(o, x, y, QA[s & 3u]);

@@ -102,11 +102,16 @@ class Twin:
                     for tx in range(colour & 1, NT, 2):
                         tile_id = ty * NT + tx
                         for s in range(T * T):
-                            # steps 4b..4b+3: site words = call b, accept words = call b + 2^31 (S3)
+                            # DESIGN.md S3: a site word is a base-T*T fraction with two digits; step s uses digit
+                            # s % 2 of word (s // 2) % 4 of call s // 8; accept word = word s % 4 of call s // 4 + 2^31
+                            if s % 8 == 0:
+                                sites = philox4x32_10((s // 8, tile_id, m, self.replica), self.key)
                             if s % 4 == 0:
-                                sites = philox4x32_10((s // 4, tile_id, m, self.replica), self.key)
                                 accepts = philox4x32_10((s // 4 + 0x80000000, tile_id, m, self.replica), self.key)
-                            idx = mulhi32(sites[s % 4], T * T)
+                            word = sites[(s // 2) % 4]
+                            if s % 2 == 1:
+                                word = (word * T * T) & MASK
+                            idx = mulhi32(word, T * T)
                             x = (ox + tx * T + idx % T) % L
                             y = (oy + ty * T + idx // T) % L
                             self._attempt(x, y, accepts[s % 4])

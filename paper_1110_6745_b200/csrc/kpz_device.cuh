@@ -441,46 +441,47 @@ __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site
     }
 }
 
-// T*T sequential attempts of one tile (S3: steps 4c..4c+3 take their site words from call c and their accept
-// words from call c | 2^31).  Calls are generated B at a time, one batch ahead of the attempts that consume them
-// (the generator is counter-based, so the next batch does not depend on the lattice): the multiplier pipe works
-// on batch b+1 while the shared-memory round trips of batch b are in flight.
-#ifndef KPZ_PHILOX_BATCH
-#define KPZ_PHILOX_BATCH 2u
-#endif
+// T*T sequential attempts of one tile (S3).  Site call c serves steps 8c..8c+7: each of its four words is a
+// base-T*T fraction with two digits (for the power-of-two T*T of this path: its top 2*log2(T) bits and the next
+// 2*log2(T) bits).  Accept calls 2c and 2c+1 (counter | 2^31) serve the same eight steps, one word each, and are
+// evaluated only in MODE 1.  Calls are generated one batch ahead of the attempts that consume them (the generator
+// is counter-based, so the next batch does not depend on the lattice): the multiplier pipe works on batch b+1
+// while the shared-memory round trips of batch b are in flight.
 template <int T, int NTHR, int MODE, bool TRACK>
 __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const UpdateParams& P, uint32_t tile_id,
                                                uint32_t replica, uint32_t& n_dep, uint32_t& n_rem, int32_t& dh00,
                                                uint32_t origin_idx) {
-    constexpr uint32_t CALLS = (uint32_t)(T * T) / 4u;
-    constexpr uint32_t B = (CALLS >= KPZ_PHILOX_BATCH) ? KPZ_PHILOX_BATCH : CALLS;
+    constexpr uint32_t CALLS = (uint32_t)(T * T) / 8u;
     constexpr uint32_t ACCEPT = 0x80000000u;
-    uint4 cur[B], nxt[B], cur_a[MODE ? B : 1u], nxt_a[MODE ? B : 1u];
-#pragma unroll
-    for (uint32_t k = 0; k < B; ++k) {
-        cur[k] = philox4x32_10(k, tile_id, P.m, replica, P.key);
-        if (MODE) cur_a[k] = philox4x32_10(k | ACCEPT, tile_id, P.m, replica, P.key);
+    constexpr uint32_t TT = (uint32_t)(T * T);
+    uint4 cur, nxt, cur_a[2], nxt_a[2];
+    cur = philox4x32_10(0u, tile_id, P.m, replica, P.key);
+    if (MODE) {
+        cur_a[0] = philox4x32_10(0u | ACCEPT, tile_id, P.m, replica, P.key);
+        cur_a[1] = philox4x32_10(1u | ACCEPT, tile_id, P.m, replica, P.key);
     }
 #pragma unroll 1
-    for (uint32_t c = 0; c < CALLS; c += B) {
-        // batch b+1 (the last iteration generates one unused batch: CALLS/B + 1 batches for CALLS/B used)
-#pragma unroll
-        for (uint32_t k = 0; k < B; ++k) {
-            nxt[k] = philox4x32_10(c + B + k, tile_id, P.m, replica, P.key);
-            if (MODE) nxt_a[k] = philox4x32_10((c + B + k) | ACCEPT, tile_id, P.m, replica, P.key);
+    for (uint32_t c = 0; c < CALLS; ++c) {
+        // batch c+1 (the last iteration generates one unused batch)
+        nxt = philox4x32_10(c + 1u, tile_id, P.m, replica, P.key);
+        if (MODE) {
+            nxt_a[0] = philox4x32_10((2u * c + 2u) | ACCEPT, tile_id, P.m, replica, P.key);
+            nxt_a[1] = philox4x32_10((2u * c + 3u) | ACCEPT, tile_id, P.m, replica, P.key);
         }
-#pragma unroll
-        for (uint32_t k = 0; k < B; ++k) {
-            const uint4 qa = MODE ? cur_a[k] : make_uint4(0u, 0u, 0u, 0u);
-            attempt<T, NTHR, MODE, TRACK>(sm, cur[k].x, qa.x, P, n_dep, n_rem, dh00, origin_idx);
-            attempt<T, NTHR, MODE, TRACK>(sm, cur[k].y, qa.y, P, n_dep, n_rem, dh00, origin_idx);
-            attempt<T, NTHR, MODE, TRACK>(sm, cur[k].z, qa.z, P, n_dep, n_rem, dh00, origin_idx);
-            attempt<T, NTHR, MODE, TRACK>(sm, cur[k].w, qa.w, P, n_dep, n_rem, dh00, origin_idx);
-        }
-#pragma unroll
-        for (uint32_t k = 0; k < B; ++k) {
-            cur[k] = nxt[k];
-            if (MODE) cur_a[k] = nxt_a[k];
+        const uint4 a0 = MODE ? cur_a[0] : make_uint4(0u, 0u, 0u, 0u);
+        const uint4 a1 = MODE ? cur_a[1] : make_uint4(0u, 0u, 0u, 0u);
+        attempt<T, NTHR, MODE, TRACK>(sm, cur.x, a0.x, P, n_dep, n_rem, dh00, origin_idx);
+        attempt<T, NTHR, MODE, TRACK>(sm, cur.x * TT, a0.y, P, n_dep, n_rem, dh00, origin_idx);
+        attempt<T, NTHR, MODE, TRACK>(sm, cur.y, a0.z, P, n_dep, n_rem, dh00, origin_idx);
+        attempt<T, NTHR, MODE, TRACK>(sm, cur.y * TT, a0.w, P, n_dep, n_rem, dh00, origin_idx);
+        attempt<T, NTHR, MODE, TRACK>(sm, cur.z, a1.x, P, n_dep, n_rem, dh00, origin_idx);
+        attempt<T, NTHR, MODE, TRACK>(sm, cur.z * TT, a1.y, P, n_dep, n_rem, dh00, origin_idx);
+        attempt<T, NTHR, MODE, TRACK>(sm, cur.w, a1.z, P, n_dep, n_rem, dh00, origin_idx);
+        attempt<T, NTHR, MODE, TRACK>(sm, cur.w * TT, a1.w, P, n_dep, n_rem, dh00, origin_idx);
+        cur = nxt;
+        if (MODE) {
+            cur_a[0] = nxt_a[0];
+            cur_a[1] = nxt_a[1];
         }
     }
 }
