@@ -30,10 +30,16 @@ UNIT = "Gupd/s"
 MCS_PER_STEP = 10
 WORKLOAD = dict(L=1 << 17, tile=64, p=1.0, q=0.0, seed=42)
 
-# Algorithmic integer work per attempted update: half a Philox4x32-10 call
-# (10 32x32->64 multiplies + 10 three-input XORs) + 16 bit-logic/address ops of the update itself.
-ALG_OPS_PER_UPDATE = 36
+# Algorithmic work per attempted update on the binding pipe, for p = 1, q = 0:
+# ALU-pipe operations (LOP3 / SHF / LEA / IADD; 16 lanes per clock per scheduler):
+#   1/8 Philox4x32-10 call = 2.5 three-input XORs  (its 2.5 32x32->64 multiplies run on the FMA pipe)
+#   + 12 for the attempt: row index, word address, parity word, own^parity, 2 neighbour alignments,
+#     site bit (2), 2 neighbour tests, mask, count.
+ALG_ALU_OPS_PER_UPDATE = 14.5
+ALG_MUL_OPS_PER_UPDATE = 2.5
 ALG_BYTES_PER_UPDATE = 0.5          # each site (2 bits) read once and written once per MCS
+# dram__bytes_read.sum + dram__bytes_write.sum of one update launch at L = 2^17 (profiles/, ncu --set full)
+TRAFFIC_BYTES_PER_LAUNCH = 6.24e9
 
 
 def _peaks():
@@ -192,13 +198,17 @@ def run_ours(args):
     upd_launch_ms = upd_ms / n_upd_launch
     upd_per_launch = L * L / 4
     sm_mhz = clocks.get("sm_mhz") or sm_max
-    # ALU peak: 148 SMs x 4 SMSPs x 32 lanes x 1 instruction/clk at the maximum SM clock
-    alu_peak_tops = 148 * 4 * 32 * sm_max * 1e6 / 1e12
-    achieved_tops = upd_per_launch * ALG_OPS_PER_UPDATE / (upd_launch_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "achieved": achieved_tops, "peak": alu_peak_tops, "unit": "Tops/s (int32 lane-ops)",
-                "frac": achieved_tops / alu_peak_tops, "traffic": None, "kernel": "kpz_update_kernel<64,32,0>",
-                "alg_ops_per_update": ALG_OPS_PER_UPDATE, "launch_ms": upd_launch_ms,
-                "peak_source": "148 SM x 128 lane-ops/clk x clocks.max.sm (issue limit; DESIGN.md)",
+    # ALU-pipe peak: 148 SMs x 4 schedulers x 16 lanes/clk at the maximum SM clock
+    alu_peak_tops = 148 * 4 * 16 * sm_max * 1e6 / 1e12
+    achieved_tops = upd_per_launch * ALG_ALU_OPS_PER_UPDATE / (upd_launch_ms * 1e-3) / 1e12
+    general = not (w["p"] >= 1.0 and w["q"] <= 0.0)
+    roofline = {"bound": "alu", "achieved": achieved_tops, "peak": alu_peak_tops, "unit": "Tops/s (ALU-pipe lane-ops)",
+                "frac": achieved_tops / alu_peak_tops, "traffic": TRAFFIC_BYTES_PER_LAUNCH if L == (1 << 17) else None,
+                "kernel": "kpz_update_kernel<%d,%d,%d>" % (T, 32 if T == 64 else 64, 1 if general else 0),
+                "alg_alu_ops_per_update": ALG_ALU_OPS_PER_UPDATE, "alg_mul_ops_per_update": ALG_MUL_OPS_PER_UPDATE,
+                "launch_ms": upd_launch_ms, "updates_per_launch": upd_per_launch,
+                "peak_source": "148 SM x 4 schedulers x 16 ALU lanes/clk x clocks.max.sm from MEASURED_PEAKS.json "
+                               "(%s); LOP3 issue interval of 2 clk per scheduler confirmed by microbenchmark (DESIGN.md)" % src,
                 "hbm": {"achieved": upd_per_launch * ALG_BYTES_PER_UPDATE / (upd_launch_ms * 1e-3) / 1e9,
                         "peak": hbm_peak, "unit": "GB/s", "peak_source": src + " MEASURED_PEAKS.json",
                         "frac": upd_per_launch * ALG_BYTES_PER_UPDATE / (upd_launch_ms * 1e-3) / 1e9 / hbm_peak}}
