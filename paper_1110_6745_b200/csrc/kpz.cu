@@ -24,8 +24,8 @@ struct ScratchLayout {
     size_t misc;      // 8 x u64    : [0] hash accumulator, [1] validation flags
     size_t base;      // [R][L] i32
     size_t cS0;       // [R][NC][L] i32
-    size_t cS1;       // [R][NC][L] i64
-    size_t cS2;       // [R][NC][L] i64
+    size_t cS1;       // [R][NC][L] i32
+    size_t cS2;       // [R][NC][L] i32
     size_t total;
     uint32_t n_chunks, rows_per_chunk;
 };
@@ -34,17 +34,9 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 ScratchLayout scratch_layout(uint32_t L, uint32_t R) {
     ScratchLayout s;
-    const uint32_t W = L / 32, colblocks = (W + 7) / 8;
-    // enough (column block x chunk x replica) CTAs to fill 148 SMs several times; chunks are multiples of 32 rows
-    uint64_t want = 148ull * 8ull;
-    uint64_t have = (uint64_t)colblocks * R;
-    uint32_t nc = (uint32_t)((want + have - 1) / have);
-    uint32_t max_nc = L / 32;
-    if (nc > max_nc) nc = max_nc;
-    if (nc < 1) nc = 1;
-    uint32_t rpc = (L + nc - 1) / nc;
-    rpc = (rpc + 31) / 32 * 32;
-    nc = (L + rpc - 1) / rpc;
+    // chunks of at most 1024 rows (multiple of 32): chunk-relative sums then fit 32 bits (kpz_column_chunk_kernel)
+    uint32_t rpc = L < 1024u ? L : 1024u;
+    uint32_t nc = (L + rpc - 1) / rpc;
     s.n_chunks = nc;
     s.rows_per_chunk = rpc;
     size_t o = 0;
@@ -53,8 +45,8 @@ ScratchLayout scratch_layout(uint32_t L, uint32_t R) {
     s.misc = o;  o += 256;
     s.base = o;  o += align_up((size_t)R * L * 4, 256);
     s.cS0 = o;   o += align_up((size_t)R * nc * L * 4, 256);
-    s.cS1 = o;   o += align_up((size_t)R * nc * L * 8, 256);
-    s.cS2 = o;   o += align_up((size_t)R * nc * L * 8, 256);
+    s.cS1 = o;   o += align_up((size_t)R * nc * L * 4, 256);
+    s.cS2 = o;   o += align_up((size_t)R * nc * L * 4, 256);
     s.total = o;
     return s;
 }
@@ -188,15 +180,15 @@ int32_t measure_relative(kpz_ctx* c, std::vector<i128>& S1, std::vector<i128>& S
     unsigned long long* msum = reinterpret_cast<unsigned long long*>(sc + c->sl.msum);
     int32_t* base = reinterpret_cast<int32_t*>(sc + c->sl.base);
     int32_t* cS0 = reinterpret_cast<int32_t*>(sc + c->sl.cS0);
-    long long* cS1 = reinterpret_cast<long long*>(sc + c->sl.cS1);
-    long long* cS2 = reinterpret_cast<long long*>(sc + c->sl.cS2);
+    int32_t* cS1 = reinterpret_cast<int32_t*>(sc + c->sl.cS1);
+    int32_t* cS2 = reinterpret_cast<int32_t*>(sc + c->sl.cS2);
     KPZ_CUDA(c, cudaMemsetAsync(msum, 0, (size_t)R * 32, c->stream));
     int nthr = 1024;
     while (nthr > 32 && (uint32_t)nthr > L) nthr >>= 1;
     kpz::kpz_row0_prefix_kernel<<<R, nthr, 0, c->stream>>>(c->d_lattice, plane_words, L, W, base);
     KPZ_CUDA(c, cudaGetLastError());
-    dim3 g1((W + 7) / 8, c->sl.n_chunks, R);
-    kpz::kpz_column_chunk_kernel<<<g1, 256, 0, c->stream>>>(c->d_lattice, plane_words, L, W, c->sl.rows_per_chunk, cS0,
+    dim3 g1((W + 127) / 128, c->sl.n_chunks, R);
+    kpz::kpz_column_chunk_kernel<<<g1, 128, 0, c->stream>>>(c->d_lattice, plane_words, L, W, c->sl.rows_per_chunk, cS0,
                                                          cS1, cS2);
     KPZ_CUDA(c, cudaGetLastError());
     dim3 g2((L + 255) / 256, R);

@@ -620,47 +620,99 @@ __global__ void kpz_row0_prefix_kernel(const uint32_t* __restrict__ lattice, uin
     }
 }
 
-// grid (ceil(W/8), n_chunks, R), block 256: warp w of the block owns word-column 8*blockIdx.x + w, lane = bit.
-__global__ void __launch_bounds__(256) kpz_column_chunk_kernel(const uint32_t* __restrict__ lattice,
+// Column-chunk kernel.  grid (ceil(W/128), n_chunks, R), block 128: one THREAD owns one word-column (32 columns)
+// of one chunk of rows_per_chunk <= 1024 rows (a multiple of 32).  Per 32 rows it loads 32 words (coalesced across
+// the lanes of a warp), transposes the 32x32 bit block in registers so that each column becomes one word (bit k =
+// row k), and walks every column 8 rows at a time through a 256-entry table in shared memory: a byte b of sigma_y
+// bits (bit k set <=> step +1) has exit S0 = l_7, S1 = sum l_k, S2 = sum l_k^2 with l_k = sum_{j<=k} (+-1), and a
+// leaf of n = 8 rows entered at height B contributes n*B + S1 and n*B^2 + 2*B*S1 + S2.  Row 0 of the lattice
+// carries no sigma_y step (eq. 3): chunk 0 is walked as if it did and corrected per column afterwards
+// (l = l' - s0:  sum l = sum l' - n*s0,  sum l^2 = sum l'^2 - 2*s0*sum l' + n).
+// All chunk-relative sums fit 32 bits: |l| <= 1024, sum l^2 <= 2^30.
+__device__ __forceinline__ void transpose32x32(uint32_t (&a)[32]) {
+    // after the call: bit k of a[c] = bit c of the former a[k]
+#pragma unroll
+    for (int j = 16, it = 0; it < 5; ++it, j >>= 1) {
+        const uint32_t m = (j == 16) ? 0x0000FFFFu : (j == 8) ? 0x00FF00FFu : (j == 4) ? 0x0F0F0F0Fu
+                         : (j == 2) ? 0x33333333u : 0x55555555u;
+#pragma unroll
+        for (int k = 0; k < 32; ++k) {
+            if ((k & j) == 0) {
+                const uint32_t t = ((a[k] >> j) ^ a[k + j]) & m;
+                a[k] ^= t << j;
+                a[k + j] ^= t;
+            }
+        }
+    }
+}
+
+__global__ void __launch_bounds__(128) kpz_column_chunk_kernel(const uint32_t* __restrict__ lattice,
                                                                uint64_t plane_words, uint32_t L, uint32_t W,
                                                                uint32_t rows_per_chunk, int32_t* __restrict__ cS0,
-                                                               long long* __restrict__ cS1,
-                                                               long long* __restrict__ cS2) {
-    const uint32_t lane = threadIdx.x & 31u;
-    const uint32_t wcol = blockIdx.x * 8u + (threadIdx.x >> 5);
+                                                               int32_t* __restrict__ cS1, int32_t* __restrict__ cS2) {
+    __shared__ uint32_t lut[256];      // (S0 & 0xFF) | (S1 & 0xFF) << 8 | S2 << 16
+    for (uint32_t b = threadIdx.x; b < 256u; b += blockDim.x) {
+        int l = 0, s1 = 0, s2 = 0;
+        for (int k = 0; k < 8; ++k) {
+            l += ((b >> k) & 1u) ? 1 : -1;
+            s1 += l;
+            s2 += l * l;
+        }
+        lut[b] = ((uint32_t)l & 0xFFu) | (((uint32_t)s1 & 0xFFu) << 8) | ((uint32_t)s2 << 16);
+    }
+    __syncthreads();
+    const uint32_t wcol = blockIdx.x * 128u + threadIdx.x;
     if (wcol >= W) return;
     const uint32_t chunk = blockIdx.y, replica = blockIdx.z, n_chunks = gridDim.y;
     const uint32_t* planeY = lattice + (size_t)replica * 2u * plane_words + plane_words;
     const uint32_t y_begin = chunk * rows_per_chunk;
     const uint32_t y_end = min(L, y_begin + rows_per_chunk);
-    int32_t l = 0;
-    long long s1 = 0, s2 = 0;
+    int32_t B[32], s1[32], s2[32];
+#pragma unroll
+    for (int c = 0; c < 32; ++c) { B[c] = 0; s1[c] = 0; s2[c] = 0; }
+    uint32_t first_row = 0u;
+#pragma unroll 1
     for (uint32_t yb = y_begin; yb < y_end; yb += 32u) {
-        // lane k fetches the word of row yb+k; rows are then consumed in order via shuffles
-        const uint32_t yr = yb + lane;
-        const uint32_t mine = (yr < y_end) ? __ldg(planeY + (size_t)yr * W + wcol) : 0u;
-        const uint32_t nrow = min(32u, y_end - yb);
-        int32_t t1 = 0;
-        for (uint32_t k = 0; k < nrow; ++k) {
-            const uint32_t word = __shfl_sync(0xFFFFFFFFu, mine, (int)k);
-            const int32_t sig = (int32_t)(((word >> lane) & 1u) << 1) - 1;
-            if (yb + k > 0u) l += sig;                       // row 0 carries no sigma_y step (eq. 3)
-            t1 += l;
-            s2 += (long long)l * (long long)l;
+        uint32_t a[32];
+#pragma unroll
+        for (int k = 0; k < 32; ++k) a[k] = __ldg(planeY + (size_t)(yb + (uint32_t)k) * W + wcol);
+        if (yb == 0u) first_row = a[0];
+        transpose32x32(a);
+#pragma unroll
+        for (int c = 0; c < 32; ++c) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const uint32_t e = lut[(a[c] >> (8 * q)) & 0xFFu];
+                const int32_t S0 = (int32_t)(int8_t)(e & 0xFFu), S1 = (int32_t)(int8_t)((e >> 8) & 0xFFu);
+                const int32_t S2 = (int32_t)(e >> 16);
+                const int32_t t = 8 * B[c] + S1;
+                s1[c] += t;
+                s2[c] += B[c] * (t + S1) + S2;
+                B[c] += S0;
+            }
         }
-        s1 += t1;
     }
-    const size_t o = ((size_t)replica * n_chunks + chunk) * L + (size_t)wcol * 32u + lane;
-    cS0[o] = l;
-    cS1[o] = s1;
-    cS2[o] = s2;
+    const int32_t n = (int32_t)(y_end - y_begin);
+    const size_t o = ((size_t)replica * n_chunks + chunk) * L + (size_t)wcol * 32u;
+#pragma unroll
+    for (int c = 0; c < 32; ++c) {
+        if (chunk == 0u) {
+            const int32_t s0 = ((first_row >> c) & 1u) ? 1 : -1;
+            s2[c] += -2 * s0 * s1[c] + n;
+            s1[c] -= n * s0;
+            B[c] -= s0;
+        }
+        cS0[o + c] = B[c];
+        cS1[o + c] = s1[c];
+        cS2[o + c] = s2[c];
+    }
 }
 
 // grid (ceil(L/256), R), block 256: one thread per column; out[replica][4] += {lo(S1), hi(S1), lo(S2), hi(S2)}
 __global__ void __launch_bounds__(256) kpz_combine_kernel(const int32_t* __restrict__ base,
                                                           const int32_t* __restrict__ cS0,
-                                                          const long long* __restrict__ cS1,
-                                                          const long long* __restrict__ cS2, uint32_t L,
+                                                          const int32_t* __restrict__ cS1,
+                                                          const int32_t* __restrict__ cS2, uint32_t L,
                                                           uint32_t n_chunks, uint32_t rows_per_chunk,
                                                           unsigned long long* __restrict__ msum) {
     const uint32_t replica = blockIdx.y;
