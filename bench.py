@@ -103,9 +103,8 @@ def run_ours(args):
     import torch
     import paper_1110_6745_b200 as pkg
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_1110_6745_b200 import shard
+    rank, world, local = shard.rank_world()
     dist = None
     if world > 1:
         import torch.distributed as dist
@@ -118,7 +117,7 @@ def run_ours(args):
         w["L"] = args.L
     L, T = w["L"], w["tile"]
     # weak scaling: every rank advances its own independent lattice (replica id = rank in the Philox counter)
-    k = pkg.KPZ(L, w["p"], w["q"], T, w["seed"] + rank, device=dev)
+    k = pkg.KPZ(L, w["p"], w["q"], T, shard.rank_seed(w["seed"], rank), device=dev)
     k.init_flat()
     att_per_step = MCS_PER_STEP * L * L
 
@@ -156,11 +155,10 @@ def run_ours(args):
     launches = k.launch_count() - launches0
     upd_ms = sum(a.elapsed_time(b) for a, b, _ in ev)
     meas_ms = sum(b.elapsed_time(c) for _, b, c in ev)
-    if dist is not None:
-        tt = torch.tensor([ms_total], device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms_total = float(tt.item())
-    value = world * args.steps * att_per_step / (ms_total * 1e-3) / 1e9
+    # whole job: units of all ranks / max over ranks of the device time
+    _, sec_total, rate = shard.aggregate(args.steps * att_per_step, ms_total * 1e-3, device=dev)
+    ms_total = sec_total * 1e3
+    value = rate / 1e9
 
     # ---- end to end through the C ABI with HOST buffers (kpz_step_host), copies inside the timed region ----
     e2e = None
@@ -180,11 +178,8 @@ def run_ours(args):
             mcs_now += MCS_PER_STEP
         torch.cuda.synchronize()
         e2e_s = time.perf_counter() - w0
-        if dist is not None:
-            tt = torch.tensor([e2e_s], device=dev)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            e2e_s = float(tt.item())
-        e2e = {"value": world * n_e2e * att_per_step / e2e_s / 1e9, "unit": UNIT,
+        _, e2e_s, e2e_rate = shard.aggregate(n_e2e * att_per_step, e2e_s, device=dev)
+        e2e = {"value": e2e_rate / 1e9, "unit": UNIT,
                "h2d_bytes_per_step": k.lattice_bytes + 8, "d2h_bytes_per_step": k.lattice_bytes + 3 * 8 + 32,
                "steps": n_e2e, "api": "kpz_step_host (pinned host lattice in/out)"}
     except Exception as exc:   # e.g. not enough pinned host memory on the box
