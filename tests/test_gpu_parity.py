@@ -290,8 +290,9 @@ def test_config3_full_size_windows_and_invariants(pkg):
 
 
 def test_config5_shape_general_pq(pkg):
-    """BASELINE config 5 parameters (p=0.75, q=0.25, T=64, seed 3): full parity at L=8192, windows at L=2^19
-    when KPZ_TEST_2P19=1 (64 GiB of HBM)."""
+    """BASELINE config 5 parameters (p=0.75, q=0.25, T=64, seed 3): full parity at L=8192, then the config itself
+    (L=2^19, 64 GiB packed) with sampled windows vs the light-cone window oracle and the global invariants,
+    whenever the GPU has the memory (KPZ_TEST_2P19=0 skips it)."""
     import torch
     L, T, seed = 8192, 64, 3
     k = pkg.KPZ(L, 0.75, 0.25, T, seed)
@@ -304,7 +305,8 @@ def test_config5_shape_general_pq(pkg):
         assert k.state_hash() == o.state_hash()
     _compare_full(k, o)
     k.close()
-    if os.environ.get("KPZ_TEST_2P19", "0") == "1":
+    free_bytes, _ = torch.cuda.mem_get_info()
+    if os.environ.get("KPZ_TEST_2P19", "1") == "1" and free_bytes > 72 * 2**30:
         torch.cuda.empty_cache()
         L, n = 1 << 19, 2
         k = pkg.KPZ(L, 0.75, 0.25, T, seed)
