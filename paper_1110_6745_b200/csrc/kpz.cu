@@ -134,8 +134,9 @@ int32_t launch_update_t(kpz_ctx* c, const kpz::UpdateParams& P) {
 
 template <int T, int NTHR>
 int32_t launch_update_mode(kpz_ctx* c, const kpz::UpdateParams& P) {
-    const bool simple = (c->p >= 1.0 && c->q <= 0.0);
-    return simple ? launch_update_t<T, NTHR, 0>(c, P) : launch_update_t<T, NTHR, 1>(c, P);
+    if (c->p >= 1.0 && c->q <= 0.0) return launch_update_t<T, NTHR, 0>(c, P);
+    if (P.thr_p >= 1 && P.thr_q >= 1) return launch_update_t<T, NTHR, 1>(c, P);
+    return launch_update_t<T, NTHR, 2>(c, P);
 }
 
 int32_t launch_update(kpz_ctx* c, uint32_t m, uint32_t slot) {
@@ -152,6 +153,8 @@ int32_t launch_update(kpz_ctx* c, uint32_t m, uint32_t slot) {
     P.blocked = (P.HN % 8 == 0) ? 1u : 0u;
     P.thr_p = accept_threshold(c->p);
     P.thr_q = accept_threshold(c->q);
+    P.tp_incl = (uint32_t)(P.thr_p - 1);
+    P.tq_incl = (uint32_t)(P.thr_q - 1);
     P.m = m;
     P.slot = slot;
     P.key.k0 = (uint32_t)(c->seed & 0xFFFFFFFFull);

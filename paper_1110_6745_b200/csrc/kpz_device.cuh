@@ -60,6 +60,7 @@ struct UpdateParams {
     uint64_t plane_words;          // L*L/32
     uint64_t total_items;          // R * HN*HN  (tiles of one colour over all replicas)
     uint64_t thr_p, thr_q;         // accept iff (uint64)word < thr
+    uint32_t tp_incl, tq_incl;     // thr - 1 (MODE 1: both thresholds >= 1, accept iff word <= thr - 1)
     uint32_t L, NT, HN;            // lattice edge, tiles per edge, NT/2
     uint32_t W;                    // L/32: words per bit-line
     uint32_t tiles_per_colour;     // HN*HN
@@ -373,7 +374,7 @@ __device__ __forceinline__ void stage_out_narrow(uint32_t* __restrict__ planeX, 
 }
 
 // ---- a4: one attempt (eq. 2).  MODE 0: p = 1, q = 0 (accept words are never needed and their Philox calls are
-// never evaluated -- bit-identical, the generator is counter-based).  MODE 1: general p, q.  TRACK: this
+// never evaluated -- bit-identical, the generator is counter-based).  MODE 1: p, q both > 0.  MODE 2: any p, q.  TRACK: this
 // thread's tile holds global site (0,0) at local index origin_idx.  A flip is one shared-memory XOR reduction
 // (ATOMS.XOR without return) with a zero mask when nothing flips: no branch on the outcome, so a whole batch of
 // attempts stays one basic block for the instruction scheduler.
@@ -385,6 +386,11 @@ __device__ __forceinline__ uint32_t lop3_any_differs(uint32_t v, uint32_t a, uin
 __device__ __forceinline__ uint32_t lop3_all_differ(uint32_t v, uint32_t a, uint32_t b) {
     uint32_t r;   // (v ^ a) & (v ^ b)
     asm("lop3.b32 %0, %1, %2, %3, 0x18;" : "=r"(r) : "r"(v), "r"(a), "r"(b));
+    return r;
+}
+__device__ __forceinline__ uint32_t lop3_and3(uint32_t m, uint32_t x, uint32_t y) {
+    uint32_t r;   // m & x & y
+    asm("lop3.b32 %0, %1, %2, %3, 0x80;" : "=r"(r) : "r"(m), "r"(x), "r"(y));
     return r;
 }
 __device__ __forceinline__ uint32_t lop3_and_not_not(uint32_t m, uint32_t x, uint32_t y) {
@@ -429,9 +435,20 @@ __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site
         atomicXor(a, md0);
         n_dep += (md0 != 0u) ? 1u : 0u;
         if (TRACK) dh00 += (md0 != 0u && idx == origin_idx) ? 2 : 0;
+    } else if (MODE == 1) {
+        // both probabilities > 0: 32-bit inclusive thresholds.  A site is a minimum or a maximum, never both: the
+        // threshold is chosen by the site type, one compare decides.
+        const uint32_t mr0 = lop3_and3(bit, lop3_all_differ(v, wl, wr), lop3_all_differ(v, wd, wu));
+        const bool is_min = md0 != 0u;
+        const bool ok = accept_word <= (is_min ? P.tp_incl : P.tq_incl);
+        const uint32_t m = ok ? (md0 | mr0) : 0u;
+        atomicXor(a, m);
+        n_dep += (ok && is_min) ? 1u : 0u;
+        n_rem += (m != 0u && !is_min) ? 1u : 0u;
+        if (TRACK) dh00 += (idx == origin_idx && m != 0u) ? (is_min ? 2 : -2) : 0;
     } else {
-        // local maximum <=> every neighbour differs from v
-        const uint32_t mr0 = bit & lop3_all_differ(v, wl, wr) & lop3_all_differ(v, wd, wu);
+        // general thresholds (a probability of exactly 0 with the other one in (0,1])
+        const uint32_t mr0 = lop3_and3(bit, lop3_all_differ(v, wl, wr), lop3_all_differ(v, wd, wu));
         const uint32_t md = ((uint64_t)accept_word < P.thr_p) ? md0 : 0u;
         const uint32_t mr = ((uint64_t)accept_word < P.thr_q) ? mr0 : 0u;
         atomicXor(a, md | mr);

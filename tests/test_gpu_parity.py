@@ -148,6 +148,9 @@ def _compare_scalars(k, os_, replica_slice=None):
     (1024, 64, 1.0, 0.0, 10, 4),       # HN = 8 -> blocked lane mapping
     (1024, 32, 0.6, 0.1, 11, 3),
     (1024, 16, 1.0, 0.0, 12, 3),
+    (64, 16, 0.5, 0.0, 13, 4),         # a probability of exactly 0: the 64-bit threshold path
+    (128, 64, 0.0, 0.7, 14, 3),
+    (128, 32, 1.0, 0.4, 15, 3),        # p = 1 with removals: inclusive 32-bit threshold 2^32 - 1
 ])
 def test_update_parity_every_mcs(pkg, L, T, p, q, seed, n):
     k = pkg.KPZ(L, p, q, T, seed)
