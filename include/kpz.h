@@ -133,6 +133,20 @@ int32_t kpz_import_packed(kpz_ctx* ctx, const void* host_src, size_t bytes, cons
 int32_t kpz_step_host(kpz_ctx* ctx, void* host_lattice, size_t bytes, int64_t* h00_inout, uint64_t mcs_start,
                       uint64_t mcs, int64_t* sum_h, int64_t* sum_h2, double* W2);
 
+/* ---- power spectrum along the lattice axes (eq. 15-16) ---------------- */
+
+/* Exact integer profiles of replica `replica`: col_sums[x] = sum_y h(x,y), row_sums[y] = sum_x h(x,y) with absolute
+ * heights (anchored by h(0,0) like kpz_measure).  HOST out-arrays of length L (either may be NULL).  Synchronises.
+ * Any valid L.  These are the only functions of the surface the axis modes of h(k) depend on. */
+int32_t kpz_profiles(kpz_ctx* ctx, uint32_t replica, int64_t* col_sums, int64_t* row_sums);
+
+/* Power spectrum S(k) = |h(k)|^2, h(k) = (1/L) sum_x [h(x) - <h>] exp(i k.x) (eq. 15-16 with d = 2), on the two
+ * lattice axes, k = 2 pi n / L, n = 0 .. L/2:  Sx[n] = S(k,0), Sy[n] = S(0,k) and their average S[n] ("averaging
+ * over x and y directions").  S[0] = 0.  HOST out-arrays of length L/2 + 1 (any may be NULL); one replica,
+ * one time: ensemble averages are the caller's sum.  fp64 radix-2 FFT of the two integer profiles on the device.
+ * L must be a power of two (KPZ_EINVAL otherwise).  Synchronises.  Does not modify the lattice. */
+int32_t kpz_power_spectrum(kpz_ctx* ctx, uint32_t replica, double* S, double* Sx, double* Sy);
+
 /* Number of kernels this handle has launched since creation (for bench.py "gpu_launches"). */
 int32_t kpz_launch_count(const kpz_ctx* ctx, uint64_t* out);
 

@@ -21,7 +21,7 @@ exported_symbols = [
     "kpz_workspace_bytes", "kpz_create", "kpz_create_batch", "kpz_bind", "kpz_init_flat", "kpz_run", "kpz_measure",
     "kpz_destroy", "kpz_synchronize", "kpz_last_error", "kpz_get_slopes", "kpz_get_window", "kpz_set_slopes",
     "kpz_state_hash", "kpz_counters", "kpz_export_packed", "kpz_import_packed", "kpz_step_host",
-    "kpz_launch_count", "kpz_philox_selftest",
+    "kpz_launch_count", "kpz_philox_selftest", "kpz_profiles", "kpz_power_spectrum",
 ]
 
 
@@ -57,6 +57,8 @@ def load_library() -> ctypes.CDLL:
         "kpz_set_slopes": [vp, u32, vp, vp, i64],
         "kpz_state_hash": [vp, u32, vp],
         "kpz_counters": [vp, u32, vp, vp, vp, vp, vp],
+        "kpz_profiles": [vp, u32, vp, vp],
+        "kpz_power_spectrum": [vp, u32, vp, vp, vp],
         "kpz_export_packed": [vp, vp, sz],
         "kpz_import_packed": [vp, vp, sz, vp, u64],
         "kpz_step_host": [vp, vp, sz, vp, u64, u64, vp, vp, vp],
@@ -162,6 +164,20 @@ class KPZ:
         if sx.shape != (self.L, self.L) or sy.shape != (self.L, self.L):
             raise ValueError("slope arrays must be L x L")
         self._check(self._lib.kpz_set_slopes(self._h, replica, sx.ctypes.data, sy.ctypes.data, int(h00)))
+
+    def profiles(self, replica=0):
+        """kpz_profiles: exact (col_sums[x] = sum_y h, row_sums[y] = sum_x h), int64 arrays of length L."""
+        c = np.empty(self.L, dtype=np.int64)
+        r = np.empty(self.L, dtype=np.int64)
+        self._check(self._lib.kpz_profiles(self._h, replica, c.ctypes.data, r.ctypes.data))
+        return c, r
+
+    def power_spectrum(self, replica=0):
+        """kpz_power_spectrum: (S, Sx, Sy), float64 arrays of length L/2 + 1 (k = 2 pi n / L)."""
+        n = self.L // 2 + 1
+        S, Sx, Sy = (np.empty(n, dtype=np.float64) for _ in range(3))
+        self._check(self._lib.kpz_power_spectrum(self._h, replica, S.ctypes.data, Sx.ctypes.data, Sy.ctypes.data))
+        return S, Sx, Sy
 
     def state_hash(self, replica=0):
         out = ctypes.c_uint64()

@@ -26,6 +26,12 @@ struct ScratchLayout {
     size_t cS0;       // [R][NC][L] i32
     size_t cS1;       // [R][NC][L] i32
     size_t cS2;       // [R][NC][L] i32
+    size_t colsum;    // [L] i64       column sums of one replica (power spectrum / profiles)
+    size_t rowinc;    // [L] i32
+    size_t prof;      // [2][L] i64    column and row profiles relative to h00
+    size_t fft;       // [2][L] double2
+    size_t sdir;      // [2][L/2+1] double
+    size_t savg;      // [L/2+1] double
     size_t total;
     uint32_t n_chunks, rows_per_chunk;
 };
@@ -47,6 +53,12 @@ ScratchLayout scratch_layout(uint32_t L, uint32_t R) {
     s.cS0 = o;   o += align_up((size_t)R * nc * L * 4, 256);
     s.cS1 = o;   o += align_up((size_t)R * nc * L * 4, 256);
     s.cS2 = o;   o += align_up((size_t)R * nc * L * 4, 256);
+    s.colsum = o; o += align_up((size_t)L * 8, 256);
+    s.rowinc = o; o += align_up((size_t)L * 4, 256);
+    s.prof = o;   o += align_up((size_t)2 * L * 8, 256);
+    s.fft = o;    o += align_up((size_t)2 * L * 16, 256);
+    s.sdir = o;   o += align_up((size_t)2 * (L / 2 + 1) * 8, 256);
+    s.savg = o;   o += align_up((size_t)(L / 2 + 1) * 8, 256);
     s.total = o;
     return s;
 }
@@ -176,7 +188,8 @@ int32_t require_bound(kpz_ctx* c) {
 }
 
 // sums for all replicas -> host vectors (relative to h(0,0)) + h00
-int32_t measure_relative(kpz_ctx* c, std::vector<i128>& S1, std::vector<i128>& S2, std::vector<long long>& h00) {
+int32_t measure_relative(kpz_ctx* c, std::vector<i128>& S1, std::vector<i128>& S2, std::vector<long long>& h00,
+                         bool want_colsum = false, uint32_t colsum_replica = 0) {
     const uint32_t L = c->L, R = c->R, W = L / 32;
     const uint64_t plane_words = (uint64_t)L * L / 32;
     unsigned char* sc = c->d_scratch;
@@ -195,7 +208,9 @@ int32_t measure_relative(kpz_ctx* c, std::vector<i128>& S1, std::vector<i128>& S
                                                          cS1, cS2);
     KPZ_CUDA(c, cudaGetLastError());
     dim3 g2((L + 255) / 256, R);
-    kpz::kpz_combine_kernel<<<g2, 256, 0, c->stream>>>(base, cS0, cS1, cS2, L, c->sl.n_chunks, c->sl.rows_per_chunk, msum);
+    kpz::kpz_combine_kernel<<<g2, 256, 0, c->stream>>>(base, cS0, cS1, cS2, L, c->sl.n_chunks, c->sl.rows_per_chunk, msum,
+                                                    want_colsum ? reinterpret_cast<long long*>(sc + c->sl.colsum) : nullptr,
+                                                    colsum_replica);
     KPZ_CUDA(c, cudaGetLastError());
     c->launches += 3;
     std::vector<unsigned long long> hm((size_t)R * 4), hs((size_t)R * 4);
@@ -467,6 +482,71 @@ int32_t kpz_step_host(kpz_ctx* c, void* host_lattice, size_t bytes, int64_t* h00
         }
     }
     return rc;
+}
+
+// profiles of replica `replica` relative to h00 on the device (scratch prof[2][L]) + spectra; shared by the two calls
+static int32_t run_profiles(kpz_ctx* c, uint32_t replica, bool with_fft, long long* h00_out) {
+    const uint32_t L = c->L, W = L / 32;
+    uint32_t logL = 0;
+    while ((1u << logL) < L) ++logL;
+    if (with_fft && (1u << logL) != L) return fail(c, KPZ_EINVAL, "the power spectrum needs L to be a power of two");
+    std::vector<i128> S1, S2;
+    std::vector<long long> h00;
+    int32_t rc = measure_relative(c, S1, S2, h00, true, replica);
+    if (rc != KPZ_OK) return rc;
+    *h00_out = h00[replica];
+    unsigned char* sc = c->d_scratch;
+    const uint64_t plane_words = (uint64_t)L * L / 32;
+    int32_t* inc = reinterpret_cast<int32_t*>(sc + c->sl.rowinc);
+    kpz::kpz_row_inc_kernel<<<grid_for((uint64_t)L * 32, 256), 256, 0, c->stream>>>(c->d_lattice, plane_words, replica, L, W, inc);
+    KPZ_CUDA(c, cudaGetLastError());
+    kpz::kpz_profile_fft_kernel<<<2, 1024, 0, c->stream>>>(
+        reinterpret_cast<const long long*>(sc + c->sl.colsum), reinterpret_cast<const int32_t*>(sc + c->sl.base) + (size_t)replica * L,
+        inc, reinterpret_cast<long long*>(sc + c->sl.prof), reinterpret_cast<double2*>(sc + c->sl.fft),
+        reinterpret_cast<double*>(sc + c->sl.sdir), L, with_fft ? logL : 0u);
+    KPZ_CUDA(c, cudaGetLastError());
+    c->launches += 2;
+    if (with_fft) {
+        const uint32_t n = L / 2 + 1;
+        kpz::kpz_spectrum_average_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(reinterpret_cast<const double*>(sc + c->sl.sdir),
+                                                                           reinterpret_cast<double*>(sc + c->sl.savg), n);
+        KPZ_CUDA(c, cudaGetLastError());
+        c->launches++;
+    }
+    return KPZ_OK;
+}
+
+int32_t kpz_profiles(kpz_ctx* c, uint32_t replica, int64_t* col_sums, int64_t* row_sums) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    if (replica >= c->R) return fail(c, KPZ_EINVAL, "replica out of range");
+    long long h00 = 0;
+    rc = run_profiles(c, replica, false, &h00);
+    if (rc != KPZ_OK) return rc;
+    const uint32_t L = c->L;
+    std::vector<long long> prof((size_t)2 * L);
+    KPZ_CUDA(c, cudaMemcpyAsync(prof.data(), c->d_scratch + c->sl.prof, (size_t)2 * L * 8, cudaMemcpyDeviceToHost, c->stream));
+    KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (uint32_t i = 0; i < L; ++i) {
+        if (col_sums) col_sums[i] = prof[i] + (long long)L * h00;
+        if (row_sums) row_sums[i] = prof[(size_t)L + i] + (long long)L * h00;
+    }
+    return KPZ_OK;
+}
+
+int32_t kpz_power_spectrum(kpz_ctx* c, uint32_t replica, double* S, double* Sx, double* Sy) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    if (replica >= c->R) return fail(c, KPZ_EINVAL, "replica out of range");
+    long long h00 = 0;
+    rc = run_profiles(c, replica, true, &h00);
+    if (rc != KPZ_OK) return rc;
+    const size_t n = c->L / 2 + 1;
+    if (S) KPZ_CUDA(c, cudaMemcpyAsync(S, c->d_scratch + c->sl.savg, n * 8, cudaMemcpyDeviceToHost, c->stream));
+    if (Sx) KPZ_CUDA(c, cudaMemcpyAsync(Sx, c->d_scratch + c->sl.sdir, n * 8, cudaMemcpyDeviceToHost, c->stream));
+    if (Sy) KPZ_CUDA(c, cudaMemcpyAsync(Sy, c->d_scratch + c->sl.sdir + n * 8, n * 8, cudaMemcpyDeviceToHost, c->stream));
+    KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
+    return KPZ_OK;
 }
 
 int32_t kpz_launch_count(const kpz_ctx* c, uint64_t* out) {

@@ -731,7 +731,8 @@ __global__ void __launch_bounds__(256) kpz_combine_kernel(const int32_t* __restr
                                                           const int32_t* __restrict__ cS1,
                                                           const int32_t* __restrict__ cS2, uint32_t L,
                                                           uint32_t n_chunks, uint32_t rows_per_chunk,
-                                                          unsigned long long* __restrict__ msum) {
+                                                          unsigned long long* __restrict__ msum,
+                                                          long long* __restrict__ colsum, uint32_t colsum_replica) {
     const uint32_t replica = blockIdx.y;
     const uint32_t x = blockIdx.x * 256u + threadIdx.x;
     long long a1 = 0, a2 = 0;
@@ -747,6 +748,7 @@ __global__ void __launch_bounds__(256) kpz_combine_kernel(const int32_t* __restr
             a2 += n * B * B + 2 * B * S1 + S2;
             B += cS0[o];
         }
+        if (colsum != nullptr && replica == colsum_replica) colsum[x] = a1;   // sum_y (h(x,y) - h00)
     }
     // split into 32-bit halves so that the cross-column sums cannot overflow 64 bits; warp + block reduce
     unsigned long long v[4] = {(unsigned long long)(uint32_t)a1, (unsigned long long)(a1 >> 32),
@@ -767,6 +769,116 @@ __global__ void __launch_bounds__(256) kpz_combine_kernel(const int32_t* __restr
         for (int w = 0; w < 8; ++w) t += red[w][threadIdx.x];
         atomicAdd(msum + (size_t)replica * 4u + threadIdx.x, t);
     }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Power spectrum along the two lattice axes (eq. 15-16).  With
+// h(k) = (1/L) sum_x [h(x) - <h>] exp(i k.x), the modes on the k_x axis depend on the surface only through its
+// column sums c(x) = sum_y h(x,y) and those on the k_y axis only through its row sums r(y) = sum_x h(x,y):
+// h(k_x, 0) = (1/L) sum_x c(x) exp(i k_x x).  The column sums come out of kpz_combine_kernel; the row sums are
+// r(0) = sum_x base(x) and r(y) = r(y-1) + 2*popc(row y of sigma_y) - L.  Both profiles are exact integers.
+// ------------------------------------------------------------------------------------------------------------
+// one warp per row: inc[y] = sum_x sigma_y(x,y) = 2*popc - L
+__global__ void __launch_bounds__(256) kpz_row_inc_kernel(const uint32_t* __restrict__ lattice, uint64_t plane_words,
+                                                          uint32_t replica, uint32_t L, uint32_t W,
+                                                          int32_t* __restrict__ inc) {
+    const uint32_t* planeY = lattice + (size_t)replica * 2u * plane_words + plane_words;
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
+    for (uint32_t y = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; y < L; y += warps) {
+        uint32_t c = 0;
+        for (uint32_t k = lane; k < W; k += 32u) c += __popc(__ldg(planeY + (size_t)y * W + k));
+#pragma unroll
+        for (int sft = 16; sft > 0; sft >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, sft);
+        if (lane == 0u) inc[y] = (int32_t)(2u * c) - (int32_t)L;
+    }
+}
+
+__device__ __forceinline__ long long block_sum_ll(long long v, long long* red) {
+    // sum over the 1024 threads of the block, returned to every thread
+#pragma unroll
+    for (int sft = 16; sft > 0; sft >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, sft);
+    __syncthreads();
+    if ((threadIdx.x & 31u) == 0u) red[threadIdx.x >> 5] = v;
+    __syncthreads();
+    long long t = 0;
+    for (int w = 0; w < 32; ++w) t += red[w];
+    return t;
+}
+
+// grid 2 (block 0: column profile / k_x axis, block 1: row profile / k_y axis), block 1024.  Builds the profile
+// relative to h00, removes an integer approximation of its mean (a constant only changes the k = 0 mode, which
+// is 0 by definition; removing it keeps the rounding of the transform small), runs an in-place radix-2
+// decimation-in-time FFT in fp64 on `buf` (twiddles from sincospi), and writes S(k) = |X(k)|^2 / L^2 for
+// k = 0 .. L/2.  L must be a power of two.
+__global__ void __launch_bounds__(1024) kpz_profile_fft_kernel(const long long* __restrict__ colsum,
+                                                               const int32_t* __restrict__ base,
+                                                               const int32_t* __restrict__ inc,
+                                                               long long* __restrict__ prof, double2* __restrict__ buf,
+                                                               double* __restrict__ Sdir, uint32_t L, uint32_t logL) {
+    __shared__ long long red[32];
+    __shared__ long long seg[1024];
+    const uint32_t dir = blockIdx.x, tid = threadIdx.x;
+    long long* p = prof + (size_t)dir * L;
+    double2* b = buf + (size_t)dir * L;
+    const uint32_t per = (L + 1023u) / 1024u;
+    const uint32_t i0 = tid * per, i1 = min(L, i0 + per);
+    if (dir == 0u) {
+        for (uint32_t i = tid; i < L; i += 1024u) p[i] = colsum[i];
+    } else {
+        // r(0) = sum_x base(x); r(y) = r(y-1) + inc(y): block scan over contiguous segments
+        long long sb = 0;
+        for (uint32_t i = tid; i < L; i += 1024u) sb += base[i];
+        const long long r0 = block_sum_ll(sb, red);
+        long long s = 0;
+        for (uint32_t i = i0; i < i1; ++i) s += (i == 0u) ? 0 : inc[i];
+        seg[tid] = s;
+        __syncthreads();
+        for (uint32_t d = 1; d < 1024u; d <<= 1) {
+            const long long v = (tid >= d) ? seg[tid - d] : 0;
+            __syncthreads();
+            seg[tid] += v;
+            __syncthreads();
+        }
+        long long run = r0 + seg[tid] - s;
+        for (uint32_t i = i0; i < i1; ++i) {
+            run += (i == 0u) ? 0 : inc[i];
+            p[i] = run;
+        }
+    }
+    __syncthreads();
+    if (logL == 0u) return;          // profiles only
+    long long sl = 0;
+    for (uint32_t i = tid; i < L; i += 1024u) sl += p[i];
+    const long long mean = block_sum_ll(sl, red) / (long long)L;
+    for (uint32_t i = tid; i < L; i += 1024u) {
+        const uint32_t j = __brev(i) >> (32u - logL);
+        b[j] = make_double2((double)(p[i] - mean), 0.0);
+    }
+    __syncthreads();
+    for (uint32_t s = 1; s <= logL; ++s) {
+        const uint32_t half = 1u << (s - 1u);
+        for (uint32_t t = tid; t < (L >> 1); t += 1024u) {
+            const uint32_t j = t & (half - 1u);
+            const uint32_t lo = ((t >> (s - 1u)) << s) + j, hi = lo + half;
+            double sn, cs;
+            sincospi(-(double)j / (double)half, &sn, &cs);
+            const double2 u = b[lo], v = b[hi];
+            const double2 w = make_double2(v.x * cs - v.y * sn, v.x * sn + v.y * cs);
+            b[lo] = make_double2(u.x + w.x, u.y + w.y);
+            b[hi] = make_double2(u.x - w.x, u.y - w.y);
+        }
+        __syncthreads();
+    }
+    const double inv = 1.0 / ((double)L * (double)L);
+    for (uint32_t k = tid; k <= (L >> 1); k += 1024u)
+        Sdir[(size_t)dir * ((L >> 1) + 1u) + k] = (k == 0u) ? 0.0 : (b[k].x * b[k].x + b[k].y * b[k].y) * inv;
+}
+
+// "averaging over x and y directions": S(k) = (S(k,0) + S(0,k)) / 2
+__global__ void kpz_spectrum_average_kernel(const double* __restrict__ Sdir, double* __restrict__ S, uint32_t n) {
+    const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) S[k] = 0.5 * (Sdir[k] + Sdir[n + k]);
 }
 
 // ------------------------------------------------------------------------------------------------------------

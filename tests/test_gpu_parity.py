@@ -321,3 +321,57 @@ def test_config5_shape_general_pq(pkg):
         _window_check(pkg, k, L, T, 0.75, 0.25, seed, n, 400000, 123456, 512)
         k.close()
         torch.cuda.empty_cache()
+
+
+def _spectrum_bound(prof, S_ref_dir, L):
+    """|S_gpu - S_oracle| allowed for one axis: both sides run an fp64 FFT whose
+    output error is at most delta = 4 eps log2(L) sqrt(L) ||c||_2 per mode (c = mean-free integer profile), twice
+    for the two sides; S = |X|^2 / L^2, so |dS| <= (2 |X| delta + delta^2) / L^2."""
+    c = prof.astype(np.float64) - prof.mean()
+    delta = 2 * 4 * np.finfo(np.float64).eps * np.log2(L) * np.sqrt(L) * np.linalg.norm(c)
+    X = L * np.sqrt(S_ref_dir)
+    return (2 * X * delta + delta * delta) / (L * L) + 1e-300
+
+
+@pytest.mark.parametrize("L,kind", [(64, "tri8"), (256, "raised"), (128, "stair"), (1024, "stair"), (96, "raised"),
+                                    (512, "evolved"), (2048, "evolved75")])
+def test_profiles_and_power_spectrum_parity(pkg, L, kind):
+    """kpz_profiles bit-exact against the oracle's height field; kpz_power_spectrum (1-D transforms of the two
+    profiles on the device) against the oracle's definition (2-D transform of the height field, fp64)."""
+    from oracle.spectrum import power_spectrum, profiles
+    T = 16
+    if kind in ("evolved", "evolved75"):
+        p, q = (1.0, 0.0) if kind == "evolved" else (0.75, 0.25)
+        k = pkg.KPZ(L, p, q, T, 21)
+        k.init_flat(); k.run(12)
+        o = Oracle(L, p, q, T, 21, threads=NTHREADS)
+        o.init_flat(); o.run(12)
+    else:
+        h = {"tri8": lambda: gen.triangle_heights(L, 8), "raised": lambda: gen.raised_flat_heights(L, 11, 0.4) - 5,
+             "stair": lambda: gen.staircase_heights(L, 3) + 1_000_000}[kind]()
+        sx, sy = gen.heights_to_slopes(h)
+        k = pkg.KPZ(L, 1.0, 0.0, T, 1)
+        k.init_flat(); k.set_slopes(sx, sy, h00=int(h[0, 0]))
+        o = Oracle(L, 1.0, 0.0, T, 1)
+        o.set_slopes(sx, sy, h00=int(h[0, 0]))
+    ho = o.heights().astype(np.int64)
+    oc, orow = profiles(ho)
+    gc, grow = k.profiles()
+    assert np.array_equal(gc, oc) and np.array_equal(grow, orow)
+    if L & (L - 1):
+        with pytest.raises(pkg.KpzError) as e:
+            k.power_spectrum()
+        assert e.value.code == pkg.KPZ_EINVAL
+        return
+    S, Sx, Sy = k.power_spectrum()
+    oS, oSx, oSy = power_spectrum(ho)
+    bx, by = _spectrum_bound(oc, oSx, L), _spectrum_bound(orow, oSy, L)
+    assert np.all(np.abs(Sx - oSx) <= bx), float(np.max(np.abs(Sx - oSx) / bx))
+    assert np.all(np.abs(Sy - oSy) <= by), float(np.max(np.abs(Sy - oSy) / by))
+    assert np.all(np.abs(S - oS) <= 0.5 * (bx + by))
+    assert S[0] == 0.0
+    if kind == "tri8":
+        n = L // 16                       # first harmonic of the period-16 triangle wave
+        assert abs(S[n] - (L / 16) ** 2 / np.sin(np.pi / 16) ** 4) < 1e-9 * S[n]
+    # the lattice is untouched
+    assert k.state_hash() == o.state_hash()
