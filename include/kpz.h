@@ -79,6 +79,17 @@ int32_t kpz_init_flat(kpz_ctx* ctx);
  * would pass 2^32 - 1 (it is a 32-bit Philox counter word). */
 int32_t kpz_run(kpz_ctx* ctx, uint64_t mcs);
 
+/* Chooses the domain-decomposition schedule for subsequent kpz_run calls:
+ *   KPZ_SCHEDULE_COLOURS (default): S4 -- four tile colours in random order, halo write-back, exactly L*L effective
+ *     attempts per MCS, 4 kernel launches per MCS;
+ *   KPZ_SCHEDULE_DEAD_BORDER: S5 -- the paper's own device-level scheme: every tile in one pass (1 launch
+ *     per MCS), attempts on the +x / +y edge sites of a tile do nothing ("dead borders"; a fraction 1 - (1-1/T)^2 of
+ *     the L*L attempts), same origin shift and the same Philox streams.
+ * May be called at any time between runs; KPZ_EINVAL for any other value. */
+#define KPZ_SCHEDULE_COLOURS 0
+#define KPZ_SCHEDULE_DEAD_BORDER 1
+int32_t kpz_set_schedule(kpz_ctx* ctx, int32_t schedule);
+
 /* Height reconstruction (eq. 3) and width (eq. 4).  HOST out-arrays of length n_replicas (any may be NULL).
  * sum_h, sum_h2: exact sums over all sites of h and h^2 with absolute heights anchored by h(0,0) (tracked:
  * 0 at kpz_init_flat, +-2 per accepted flip at site (0,0)).  W2 = (N*sum_h2 - sum_h^2)/N^2, N = L*L, from

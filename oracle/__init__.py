@@ -46,6 +46,8 @@ def lib() -> ctypes.CDLL:
         L.kpzo_get_threads.argtypes = [vp]
         L.kpzo_get_threads.restype = ci
         L.kpzo_init_flat.argtypes = [vp]
+        L.kpzo_set_schedule.argtypes = [vp, ci]
+        L.kpzo_set_schedule.restype = ci
         L.kpzo_run.argtypes = [vp, u64]
         L.kpzo_run.restype = ci
         L.kpzo_run_checked.argtypes = [vp, u64]
@@ -113,6 +115,11 @@ class Oracle:
     @property
     def threads(self):
         return lib().kpzo_get_threads(self._h)
+
+    def set_schedule(self, name):
+        """'colours' (S4, default) or 'dead_border' (S5, the paper's own device-level scheme)."""
+        if lib().kpzo_set_schedule(self._h, {"colours": 0, "dead_border": 1}[name]) != 0:
+            raise ValueError(name)
 
     def init_flat(self):
         lib().kpzo_init_flat(self._h)

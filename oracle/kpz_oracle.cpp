@@ -83,6 +83,7 @@ struct Oracle {
     int64_t h00;
     uint64_t mcs, attempts, deposits, removals;
     int nthreads;
+    int schedule;      // 0: four tile colours with halo (S4); 1: dead borders, one pass (S5)
 };
 
 inline bool in_window(const Oracle* o, uint32_t x, uint32_t y, size_t* idx) {
@@ -163,6 +164,9 @@ void run_tile(Oracle* o, uint32_t m, uint32_t ox, uint32_t oy, uint32_t tx, uint
         uint32_t accept_word = QA[s & 3u];
         uint32_t idx = mulhi32(site_word, steps);
         uint32_t lx = idx % T, ly = idx / T;
+        // S5: "if a thread hits a site belonging to a block border it does nothing" -- the +x and +y edge
+        // sites of a tile are the ones whose update would change slopes stored in the neighbouring tile (Fig. 1)
+        if (o->schedule == 1 && (lx == T - 1 || ly == T - 1)) continue;
         uint32_t x = (ox + tx * T + lx) % L;
         uint32_t y = (oy + ty * T + ly) % L;
         int dir = attempt(o, x, y, accept_word);
@@ -188,6 +192,22 @@ void run_one_mcs(Oracle* o) {
     uint32_t ox, oy, perm[4];
     global_draw(o, m, &ox, &oy, perm);
     const uint32_t NT = o->NT;
+    if (o->schedule == 1) {
+        // S5: every tile in one pass; the tiles are independent because their edge sites are dead
+        uint64_t n_dep = 0, n_rem = 0;
+        int64_t dh00 = 0;
+        #pragma omp parallel for collapse(2) reduction(+ : n_dep, n_rem, dh00) schedule(dynamic, 16) num_threads(o->nthreads)
+        for (int64_t ty = 0; ty < (int64_t)NT; ++ty) {
+            for (int64_t tx = 0; tx < (int64_t)NT; ++tx) {
+                if (!tile_touches_window(o, ox, oy, (uint32_t)tx, (uint32_t)ty)) continue;
+                run_tile(o, m, ox, oy, (uint32_t)tx, (uint32_t)ty, &n_dep, &n_rem, &dh00);
+            }
+        }
+        o->deposits += n_dep; o->removals += n_rem; o->h00 += dh00;
+        o->attempts += (uint64_t)o->L * o->L;
+        o->mcs += 1;
+        return;
+    }
     for (int i = 0; i < 4; ++i) {
         const uint32_t colour = perm[i];
         const uint32_t cx = colour & 1u, cy = colour >> 1;
@@ -267,6 +287,7 @@ void* kpzo_create(uint32_t L, double p, double q, uint32_t T, uint64_t seed, uin
     o->L = L; o->T = T; o->g = (T % 4 == 0) ? 4 : 1; o->NT = L / T;
     o->seed = seed; o->replica = replica; o->p = p; o->q = q;
     o->thr_p = threshold(p); o->thr_q = threshold(q);
+    o->schedule = 0;
     o->full = (ww == 0 && wh == 0);
     if (o->full) { wx0 = wy0 = 0; ww = wh = L; }
     if (ww > L || wh > L) { delete o; return nullptr; }
@@ -303,6 +324,13 @@ void kpzo_init_flat(void* h) {
             if (o->shadow) o->H[(size_t)ry * o->ww + rx] = (int32_t)((x + y) & 1u);
         }
     o->h00 = 0; o->mcs = 0; o->attempts = o->deposits = o->removals = 0;
+}
+
+// 0 = four tile colours (default), 1 = dead borders.  Returns 0, or -1 for an unknown value.
+int kpzo_set_schedule(void* h, int schedule) {
+    if (schedule != 0 && schedule != 1) return -1;
+    static_cast<Oracle*>(h)->schedule = schedule;
+    return 0;
 }
 
 int kpzo_run(void* h, uint64_t n_mcs) {

@@ -43,8 +43,9 @@ def threshold(prob):
 
 
 class Twin:
-    def __init__(self, L, p, q, T, seed, replica=0):
-        assert T >= 1 and L % (2 * T) == 0
+    def __init__(self, L, p, q, T, seed, replica=0, schedule="colours"):
+        assert T >= 1 and L % (2 * T) == 0 and schedule in ("colours", "dead_border")
+        self.schedule = schedule
         self.L, self.T, self.p, self.q, self.seed, self.replica = L, T, p, q, seed, replica
         self.g = 4 if T % 4 == 0 else 1
         self.key = (seed & MASK, (seed >> 32) & MASK)
@@ -97,9 +98,12 @@ class Twin:
         for _ in range(n_mcs):
             m = self.mcs
             ox, oy, perm = self.global_draw(m)
-            for colour in perm:
-                for ty in range(colour >> 1, NT, 2):
-                    for tx in range(colour & 1, NT, 2):
+            # S4: the four colours in the drawn order; S5 (dead borders): every tile in one pass
+            passes = [[(tx, ty) for ty in range(c >> 1, NT, 2) for tx in range(c & 1, NT, 2)] for c in perm] \
+                if self.schedule == "colours" else [[(tx, ty) for ty in range(NT) for tx in range(NT)]]
+            for tiles in passes:
+                for (tx, ty) in tiles:
+                    if True:
                         tile_id = ty * NT + tx
                         for s in range(T * T):
                             # DESIGN.md S3: a site word is a base-T*T fraction with two digits; step s uses digit
@@ -112,6 +116,8 @@ class Twin:
                             if s % 2 == 1:
                                 word = (word * T * T) & MASK
                             idx = mulhi32(word, T * T)
+                            if self.schedule == "dead_border" and (idx % T == T - 1 or idx // T == T - 1):
+                                continue      # a site on the +x / +y edge of its tile: the attempt does nothing
                             x = (ox + tx * T + idx % T) % L
                             y = (oy + ty * T + idx // T) % L
                             self._attempt(x, y, accepts[s % 4])

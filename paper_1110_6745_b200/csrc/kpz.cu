@@ -90,6 +90,7 @@ struct kpz_ctx {
     uint64_t seed;
     uint64_t mcs;            // completed MCS (all replicas advance together)
     uint64_t launches;
+    int32_t schedule;        // KPZ_SCHEDULE_COLOURS or KPZ_SCHEDULE_DEAD_BORDER
     uint32_t* d_lattice;
     unsigned char* d_scratch;
     cudaStream_t stream;
@@ -126,10 +127,10 @@ int grid_for(uint64_t n, int block, int cap = 148 * 16) {
     return (int)g;
 }
 
-template <int T, int NTHR, int MODE>
+template <int T, int NTHR, int MODE, bool DEAD>
 int32_t launch_update_t(kpz_ctx* c, const kpz::UpdateParams& P) {
     const size_t smem = (size_t)kpz::TileGeom<T>::WORDS * NTHR * sizeof(uint32_t);
-    auto kern = kpz::kpz_update_kernel<T, NTHR, MODE>;
+    auto kern = kpz::kpz_update_kernel<T, NTHR, MODE, DEAD>;
     static bool attr_set = false;
     if (!attr_set) {
         KPZ_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -144,11 +145,17 @@ int32_t launch_update_t(kpz_ctx* c, const kpz::UpdateParams& P) {
     return KPZ_OK;
 }
 
+template <int T, int NTHR, bool DEAD>
+int32_t launch_update_sched(kpz_ctx* c, const kpz::UpdateParams& P) {
+    if (c->p >= 1.0 && c->q <= 0.0) return launch_update_t<T, NTHR, 0, DEAD>(c, P);
+    if (P.thr_p >= 1 && P.thr_q >= 1) return launch_update_t<T, NTHR, 1, DEAD>(c, P);
+    return launch_update_t<T, NTHR, 2, DEAD>(c, P);
+}
+
 template <int T, int NTHR>
 int32_t launch_update_mode(kpz_ctx* c, const kpz::UpdateParams& P) {
-    if (c->p >= 1.0 && c->q <= 0.0) return launch_update_t<T, NTHR, 0>(c, P);
-    if (P.thr_p >= 1 && P.thr_q >= 1) return launch_update_t<T, NTHR, 1>(c, P);
-    return launch_update_t<T, NTHR, 2>(c, P);
+    return c->schedule == KPZ_SCHEDULE_DEAD_BORDER ? launch_update_sched<T, NTHR, true>(c, P)
+                                                   : launch_update_sched<T, NTHR, false>(c, P);
 }
 
 int32_t launch_update(kpz_ctx* c, uint32_t m, uint32_t slot) {
@@ -158,7 +165,7 @@ int32_t launch_update(kpz_ctx* c, uint32_t m, uint32_t slot) {
     P.plane_words = (uint64_t)c->L * c->L / 32;
     P.L = c->L;
     P.NT = c->L / c->T;
-    P.HN = P.NT / 2;
+    P.HN = (c->schedule == KPZ_SCHEDULE_DEAD_BORDER) ? P.NT : P.NT / 2;   // tiles per edge in one launch
     P.W = c->L / 32;
     P.tiles_per_colour = P.HN * P.HN;
     P.total_items = (uint64_t)c->R * P.tiles_per_colour;
@@ -252,7 +259,7 @@ int32_t kpz_create_batch(kpz_ctx** out, uint32_t L, double p, double q, uint32_t
     kpz_ctx* c = new (std::nothrow) kpz_ctx();
     if (!c) return KPZ_ENOMEM;
     c->L = L; c->T = tile; c->R = n_replicas; c->p = p; c->q = q; c->seed = seed;
-    c->mcs = 0; c->launches = 0;
+    c->mcs = 0; c->launches = 0; c->schedule = KPZ_SCHEDULE_COLOURS;
     c->d_lattice = nullptr; c->d_scratch = nullptr; c->stream = nullptr; c->bound = false;
     c->sl = scratch_layout(L, n_replicas);
     c->lattice_bytes = (size_t)n_replicas * ((size_t)L * L / 4);
@@ -298,12 +305,20 @@ int32_t kpz_run(kpz_ctx* c, uint64_t mcs) {
     if (c->mcs + mcs > 0xFFFFFFFFull) return fail(c, KPZ_EINVAL, "MCS clock would exceed 2^32-1");
     for (uint64_t k = 0; k < mcs; ++k) {
         const uint32_t m = (uint32_t)c->mcs;
-        for (uint32_t slot = 0; slot < 4; ++slot) {
+        const uint32_t passes = (c->schedule == KPZ_SCHEDULE_DEAD_BORDER) ? 1u : 4u;
+        for (uint32_t slot = 0; slot < passes; ++slot) {
             rc = launch_update(c, m, slot);
             if (rc != KPZ_OK) return rc;
         }
         c->mcs++;
     }
+    return KPZ_OK;
+}
+
+int32_t kpz_set_schedule(kpz_ctx* c, int32_t schedule) {
+    if (!c) return KPZ_EINVAL;
+    if (schedule != KPZ_SCHEDULE_COLOURS && schedule != KPZ_SCHEDULE_DEAD_BORDER) return fail(c, KPZ_EINVAL, "unknown schedule");
+    c->schedule = schedule;
     return KPZ_OK;
 }
 

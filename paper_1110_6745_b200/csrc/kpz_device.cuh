@@ -228,7 +228,7 @@ __device__ __forceinline__ void stage_in_wide(const uint32_t* __restrict__ plane
 // ---- a5: write back, height bits -> slopes, T >= 32.  The first and last word of a row segment are shared with
 // the (inactive, other-colour) neighbour tiles: re-read and merged.  No other thread of the launch touches
 // these words.
-template <int T, int NTHR, int NB = StageBatch<T>::N>
+template <int T, int NTHR, int NB = StageBatch<T>::N, bool DEAD = false>
 __device__ __forceinline__ void stage_out_wide(uint32_t* __restrict__ planeX, uint32_t* __restrict__ planeY, uint32_t L,
                                                uint32_t W, uint32_t x0, uint32_t y0, const uint32_t* __restrict__ sm) {
     using G = TileGeom<T>;
@@ -274,10 +274,23 @@ __device__ __forceinline__ void stage_out_wide(uint32_t* __restrict__ planeX, ui
                 uint32_t v[WPL];
 #pragma unroll
                 for (int k = 0; k < WPL; ++k) v[k] = cur[k] ^ below[k] ^ yc;
-                ly_[idx[0]] = (ey[b][0] & lowmask) | (v[0] << s);
+                if (DEAD) {
+                    // S5: every tile is active, the edge words are shared with running neighbours: apply only this
+                    // tile's own changed bits, atomically; rows 0..T-1 only
+                    if (ly < (uint32_t)T) {
+                        const uint32_t d0 = (ey[b][0] ^ (v[0] << s)) & ~lowmask;
+                        if (d0) atomicXor(ly_ + idx[0], d0);
 #pragma unroll
-                for (int k = 1; k < WPL; ++k) ly_[idx[k]] = __funnelshift_l(v[k - 1], v[k], s);
-                if (s != 0u) ly_[idx[WPL]] = (ey[b][1] & ~lowmask) | __funnelshift_l(v[WPL - 1], 0u, s);
+                        for (int k = 1; k < WPL; ++k) ly_[idx[k]] = __funnelshift_l(v[k - 1], v[k], s);
+                        const uint32_t d1 = (ey[b][1] ^ __funnelshift_l(v[WPL - 1], 0u, s)) & lowmask;
+                        if (d1) atomicXor(ly_ + idx[WPL], d1);
+                    }
+                } else {
+                    ly_[idx[0]] = (ey[b][0] & lowmask) | (v[0] << s);
+#pragma unroll
+                    for (int k = 1; k < WPL; ++k) ly_[idx[k]] = __funnelshift_l(v[k - 1], v[k], s);
+                    if (s != 0u) ly_[idx[WPL]] = (ey[b][1] & ~lowmask) | __funnelshift_l(v[WPL - 1], 0u, s);
+                }
             }
             // sigma_x(.,ly): T+1 bits (lx = 0..T) at bit offset x0; rows 0..T-1 only
             if (ly < (uint32_t)T) {
@@ -291,10 +304,20 @@ __device__ __forceinline__ void stage_out_wide(uint32_t* __restrict__ planeX, ui
                     v[k] = cur[k] ^ left ^ xc;
                 }
                 const uint32_t bitT = (hcur ^ (cur[WPL - 1] >> 31) ^ ly) & 1u;          // (T + ly) & 1 = ly & 1
-                lx_[idx[0]] = (ex[b][0] & lowmask) | (v[0] << s);
+                if (DEAD) {
+                    // S5: bits lx = 0..T-1 only (bit T is sigma_x of the right neighbour's own column 0)
+                    const uint32_t d0 = (ex[b][0] ^ (v[0] << s)) & ~lowmask;
+                    if (d0) atomicXor(lx_ + idx[0], d0);
 #pragma unroll
-                for (int k = 1; k < WPL; ++k) lx_[idx[k]] = __funnelshift_l(v[k - 1], v[k], s);
-                lx_[idx[WPL]] = (ex[b][1] & ~lowmask1) | __funnelshift_l(v[WPL - 1], 0u, s) | (bitT << s);
+                    for (int k = 1; k < WPL; ++k) lx_[idx[k]] = __funnelshift_l(v[k - 1], v[k], s);
+                    const uint32_t d1 = (ex[b][1] ^ __funnelshift_l(v[WPL - 1], 0u, s)) & lowmask;
+                    if (d1) atomicXor(lx_ + idx[WPL], d1);
+                } else {
+                    lx_[idx[0]] = (ex[b][0] & lowmask) | (v[0] << s);
+#pragma unroll
+                    for (int k = 1; k < WPL; ++k) lx_[idx[k]] = __funnelshift_l(v[k - 1], v[k], s);
+                    lx_[idx[WPL]] = (ex[b][1] & ~lowmask1) | __funnelshift_l(v[WPL - 1], 0u, s) | (bitT << s);
+                }
             }
         }
     }
@@ -354,7 +377,7 @@ __device__ __forceinline__ void stage_in_narrow(const uint32_t* __restrict__ pla
     }
 }
 
-template <int T, int NTHR>
+template <int T, int NTHR, bool DEAD>
 __device__ __forceinline__ void stage_out_narrow(uint32_t* __restrict__ planeX, uint32_t* __restrict__ planeY, uint32_t L,
                                                  uint32_t W, uint32_t x0, uint32_t y0, const uint32_t* __restrict__ sm) {
     constexpr uint32_t MT = (1u << T) - 1u;
@@ -364,11 +387,12 @@ __device__ __forceinline__ void stage_out_narrow(uint32_t* __restrict__ planeX, 
         uint32_t g = y0 + ly;
         if (g >= L) g -= L;
         const uint32_t word = sm[(ly + 1u) * NTHR], below = sm[ly * NTHR];
+        if (DEAD && ly == (uint32_t)T) break;      // S5: the +y halo row belongs to the (active) tile above
         const uint32_t sy = ((word ^ below) >> 1) ^ ycode(ly);
         store_bits(planeY + (size_t)g * W, W, x0, MT, sy);
         if (ly < (uint32_t)T) {
             const uint32_t sx = ((word ^ (word << 1)) >> 1) ^ ycode(ly);   // bit lx = h1(lx)^h1(lx-1)^h0(lx,ly), lx = 0..T
-            store_bits(planeX + (size_t)g * W, W, x0, MT1, sx);
+            store_bits(planeX + (size_t)g * W, W, x0, DEAD ? MT : MT1, sx);   // S5: bit T belongs to the right tile
         }
     }
 }
@@ -399,7 +423,7 @@ __device__ __forceinline__ uint32_t lop3_and_not_not(uint32_t m, uint32_t x, uin
     return r;
 }
 
-template <int T, int NTHR, int MODE, bool TRACK>
+template <int T, int NTHR, int MODE, bool TRACK, bool DEAD>
 __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site_word, uint32_t accept_word,
                                         const UpdateParams& P, uint32_t& n_dep, uint32_t& n_rem, int32_t& dh00,
                                         uint32_t origin_idx) {
@@ -428,7 +452,12 @@ __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site
     const uint32_t wd = *(a - G::WPR * NTHR), wu = a[G::WPR * NTHR];
     // v: bit = own_h1 ^ pi at every position of the word (rotation of 0xAAAAAAAA by the row parity)
     const uint32_t v = wo ^ __funnelshift_r(0xAAAAAAAAu, 0xAAAAAAAAu, par);
-    const uint32_t bit = __funnelshift_l(0u, 1u, sh);           // 1 << (sh & 31)
+    uint32_t bit = __funnelshift_l(0u, 1u, sh);                 // 1 << (sh & 31)
+    if (DEAD) {
+        // dead-border schedule S5: an attempt on the +x or +y edge of the tile does nothing
+        const bool edge = (((idx + 1u) & (uint32_t)(T - 1)) == 0u) || (idx >= (uint32_t)(T * (T - 1)));
+        bit = edge ? 0u : bit;
+    }
     // local minimum <=> no neighbour differs from v
     const uint32_t md0 = lop3_and_not_not(bit, lop3_any_differs(v, wl, wr), lop3_any_differs(v, wd, wu));
     if (MODE == 0) {
@@ -464,7 +493,7 @@ __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site
 // evaluated only in MODE 1.  Calls are generated one batch ahead of the attempts that consume them (the generator
 // is counter-based, so the next batch does not depend on the lattice): the multiplier pipe works on batch b+1
 // while the shared-memory round trips of batch b are in flight.
-template <int T, int NTHR, int MODE, bool TRACK>
+template <int T, int NTHR, int MODE, bool TRACK, bool DEAD>
 __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const UpdateParams& P, uint32_t tile_id,
                                                uint32_t replica, uint32_t& n_dep, uint32_t& n_rem, int32_t& dh00,
                                                uint32_t origin_idx) {
@@ -487,14 +516,14 @@ __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const 
         }
         const uint4 a0 = MODE ? cur_a[0] : make_uint4(0u, 0u, 0u, 0u);
         const uint4 a1 = MODE ? cur_a[1] : make_uint4(0u, 0u, 0u, 0u);
-        attempt<T, NTHR, MODE, TRACK>(sm, cur.x, a0.x, P, n_dep, n_rem, dh00, origin_idx);
-        attempt<T, NTHR, MODE, TRACK>(sm, cur.x * TT, a0.y, P, n_dep, n_rem, dh00, origin_idx);
-        attempt<T, NTHR, MODE, TRACK>(sm, cur.y, a0.z, P, n_dep, n_rem, dh00, origin_idx);
-        attempt<T, NTHR, MODE, TRACK>(sm, cur.y * TT, a0.w, P, n_dep, n_rem, dh00, origin_idx);
-        attempt<T, NTHR, MODE, TRACK>(sm, cur.z, a1.x, P, n_dep, n_rem, dh00, origin_idx);
-        attempt<T, NTHR, MODE, TRACK>(sm, cur.z * TT, a1.y, P, n_dep, n_rem, dh00, origin_idx);
-        attempt<T, NTHR, MODE, TRACK>(sm, cur.w, a1.z, P, n_dep, n_rem, dh00, origin_idx);
-        attempt<T, NTHR, MODE, TRACK>(sm, cur.w * TT, a1.w, P, n_dep, n_rem, dh00, origin_idx);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.x, a0.x, P, n_dep, n_rem, dh00, origin_idx);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.x * TT, a0.y, P, n_dep, n_rem, dh00, origin_idx);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.y, a0.z, P, n_dep, n_rem, dh00, origin_idx);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.y * TT, a0.w, P, n_dep, n_rem, dh00, origin_idx);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.z, a1.x, P, n_dep, n_rem, dh00, origin_idx);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.z * TT, a1.y, P, n_dep, n_rem, dh00, origin_idx);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.w, a1.z, P, n_dep, n_rem, dh00, origin_idx);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.w * TT, a1.w, P, n_dep, n_rem, dh00, origin_idx);
         cur = nxt;
         if (MODE) {
             cur_a[0] = nxt_a[0];
@@ -503,7 +532,9 @@ __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const 
     }
 }
 
-template <int T, int NTHR, int MODE>
+// DEAD = false: one colour of schedule S4 per launch (P.slot);  DEAD = true: every tile of the dead-border schedule
+// S5 in one launch (P.HN = NT).
+template <int T, int NTHR, int MODE, bool DEAD>
 __global__ void __launch_bounds__(NTHR) kpz_update_kernel(const UpdateParams P) {
     using G = TileGeom<T>;
     extern __shared__ uint32_t smem[];
@@ -528,7 +559,7 @@ __global__ void __launch_bounds__(NTHR) kpz_update_kernel(const UpdateParams P) 
     }
     uint32_t ox, oy, colour;
     global_draw<T>(P, replica, ox, oy, colour);
-    const uint32_t tx = 2u * i + (colour & 1u), ty = 2u * j + (colour >> 1);
+    const uint32_t tx = DEAD ? i : 2u * i + (colour & 1u), ty = DEAD ? j : 2u * j + (colour >> 1);
     const uint32_t X0 = ox + tx * T, Y0 = oy + ty * T;        // < L + T
     const uint32_t tile_id = ty * P.NT + tx;
     uint32_t* planeX = P.lattice + (size_t)replica * 2u * P.plane_words;
@@ -553,12 +584,12 @@ __global__ void __launch_bounds__(NTHR) kpz_update_kernel(const UpdateParams P) 
     if (active) {
         // ---- a3 + a4: T*T sequential attempts ----
         if (any_origin)
-            run_tile_steps<T, NTHR, MODE, true>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx);
+            run_tile_steps<T, NTHR, MODE, true, DEAD>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx);
         else
-            run_tile_steps<T, NTHR, MODE, false>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx);
+            run_tile_steps<T, NTHR, MODE, false, DEAD>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx);
         // ---- a5: write back ----
-        if constexpr (G::WIDE) stage_out_wide<T, NTHR>(planeX, planeY, L, W, x0, y0, sm);
-        else stage_out_narrow<T, NTHR>(planeX, planeY, L, W, x0, y0, sm);
+        if constexpr (G::WIDE) stage_out_wide<T, NTHR, StageBatch<T>::N, DEAD>(planeX, planeY, L, W, x0, y0, sm);
+        else stage_out_narrow<T, NTHR, DEAD>(planeX, planeY, L, W, x0, y0, sm);
     }
     // ---- a6: bookkeeping ----
     const uint32_t rep0 = __shfl_sync(0xFFFFFFFFu, replica, 0);

@@ -375,3 +375,72 @@ def test_profiles_and_power_spectrum_parity(pkg, L, kind):
         assert abs(S[n] - (L / 16) ** 2 / np.sin(np.pi / 16) ** 4) < 1e-9 * S[n]
     # the lattice is untouched
     assert k.state_hash() == o.state_hash()
+
+
+@pytest.mark.parametrize("L,T,p,q,seed,n", [
+    (32, 4, 1.0, 0.0, 31, 5),
+    (64, 8, 0.75, 0.25, 32, 5),
+    (96, 16, 0.5, 0.5, 33, 4),
+    (128, 32, 1.0, 0.0, 34, 5),
+    (192, 32, 0.3, 0.9, 35, 4),
+    (512, 64, 1.0, 0.0, 36, 4),
+    (1024, 64, 0.75, 0.25, 37, 3),
+    (1024, 64, 0.5, 0.0, 38, 2),
+])
+def test_dead_border_schedule_parity(pkg, L, T, p, q, seed, n):
+    """Schedule S5: every tile in one launch, +x / +y edge sites dead; bit-exact state, sums, counters."""
+    k = pkg.KPZ(L, p, q, T, seed)
+    k.set_schedule("dead_border")
+    k.init_flat()
+    o = Oracle(L, p, q, T, seed, threads=NTHREADS)
+    o.set_schedule("dead_border")
+    o.init_flat()
+    l0 = k.launch_count()
+    for t in range(n):
+        k.run(1)
+        o.run(1)
+        _compare_full(k, o)
+        _compare_scalars(k, [o])
+        assert k.state_hash() == o.state_hash()
+    # switching back to the colour schedule mid-run keeps parity (the MCS clock and the streams are shared)
+    k.set_schedule("colours"); o.set_schedule("colours")
+    k.run(1); o.run(1)
+    _compare_full(k, o)
+    _compare_scalars(k, [o])
+
+
+def test_dead_border_replicas_and_full_size_window(pkg):
+    import torch
+    L, T, R = 128, 16, 5
+    k = pkg.KPZ(L, 0.75, 0.25, T, 4, n_replicas=R)
+    k.set_schedule("dead_border")
+    k.init_flat(); k.run(3)
+    os_ = []
+    for r in range(R):
+        o = Oracle(L, 0.75, 0.25, T, 4, replica=r, threads=NTHREADS)
+        o.set_schedule("dead_border")
+        o.init_flat(); o.run(3)
+        os_.append(o)
+        _compare_full(k, o, replica=r)
+    _compare_scalars(k, os_)
+    k.close()
+    torch.cuda.empty_cache()
+    # L = 2^16 (1 GiB): one launch over 2^20 tiles; windows against the light-cone window oracle
+    L, T, seed, n = 1 << 16, 64, 9, 2
+    k = pkg.KPZ(L, 1.0, 0.0, T, seed)
+    k.set_schedule("dead_border")
+    k.init_flat(); k.run(n)
+    s1, s2, w2 = k.measure()
+    c = k.counters()
+    assert int(s1[0]) - L * L // 2 == 2 * c["deposits"] and c["removals"] == 0
+    for (wx0, wy0) in ((L - 200, L - 200), (12345, 54321)):
+        W, M = 400, 4 * (T + 1) * n
+        full = W + 2 * M
+        o = Oracle(L, 1.0, 0.0, T, seed, window=((wx0 - M) % L, (wy0 - M) % L, full, full), threads=NTHREADS)
+        o.set_schedule("dead_border")
+        o.init_flat(); o.run(n)
+        osx, osy = o.slopes()
+        gx, gy = k.get_window(wx0, wy0, W, W)
+        assert np.array_equal(gx, osx[M:M + W, M:M + W]) and np.array_equal(gy, osy[M:M + W, M:M + W])
+    k.close()
+    torch.cuda.empty_cache()

@@ -1,0 +1,65 @@
+"""Dead-border schedule S5 (the paper's own device-level scheme) in the oracle: pins."""
+import numpy as np
+import pytest
+
+from oracle import Oracle
+from oracle import kpz_twin
+
+
+@pytest.mark.parametrize("L,T,p,q,seed,n", [(16, 4, 1.0, 0.0, 5, 4), (24, 3, 0.6, 0.3, 6, 3), (32, 8, 0.75, 0.25, 7, 3),
+                                            (32, 16, 1.0, 0.0, 8, 3)])
+def test_oracle_equals_twin(L, T, p, q, seed, n):
+    o = Oracle(L, p, q, T, seed)
+    o.set_schedule("dead_border")
+    o.init_flat()
+    t = kpz_twin.Twin(L, p, q, T, seed, schedule="dead_border")
+    t.init_flat()
+    for _ in range(n):
+        o.run(1)
+        t.run(1)
+        sx, sy = o.slopes()
+        tx, ty = t.slopes()
+        assert np.array_equal(sx, np.array(tx)) and np.array_equal(sy, np.array(ty))
+        assert o.measure()[:2] == t.sums()
+        assert o.check() == 0                      # conservation, curl-free, +-1 slopes
+
+
+def test_edge_sites_of_a_tile_never_change_within_one_mcs():
+    """P:60 'conflicts at the subsystem borders are avoided simply by not updating them'; Fig. 1: two edges are
+    inactive.  Heights on the +x / +y edge of every tile of the shifted frame are unchanged by that MCS."""
+    L, T = 64, 16
+    o = Oracle(L, 1.0, 0.0, T, 3)
+    o.set_schedule("dead_border")
+    o.init_flat()
+    for m in range(6):
+        ox, oy, _ = o.global_draw(m)
+        before = o.heights().astype(np.int64)
+        o.run(1)
+        after = o.heights().astype(np.int64)
+        changed = before != after
+        xs = (np.arange(L) - ox) % T == T - 1
+        ys = (np.arange(L) - oy) % T == T - 1
+        assert not changed[:, xs].any() and not changed[ys, :].any()
+        assert changed.any()
+
+
+def test_lost_attempts_fraction_and_thread_independence():
+    """With p = 1 on the flat start of MCS 0 every attempt on a live even site flips unless an earlier flip of the
+    same MCS touched it; the count with dead borders is below the colour schedule's and results do not depend on
+    the number of OpenMP threads (tiles are independent)."""
+    L, T = 128, 16
+    res = []
+    for threads in (1, 4):
+        o = Oracle(L, 1.0, 0.0, T, 11, threads=threads)
+        o.set_schedule("dead_border")
+        o.init_flat()
+        o.run(3)
+        res.append((o.state_hash(), o.measure()[:2], o.counters()["deposits"]))
+    assert res[0] == res[1]
+    c = Oracle(L, 1.0, 0.0, T, 11)
+    c.init_flat()
+    c.run(3)
+    live = (1 - 1 / T) ** 2
+    ratio = res[0][2] / c.counters()["deposits"]
+    assert live - 0.05 < ratio < 1.0
+    assert c.counters()["attempts"] == 3 * L * L == Oracle.counters(o)["attempts"]
