@@ -10,10 +10,11 @@ import pytest
 from oracle import Oracle
 
 
-def _ensemble(L, T, p, q, runs, t_end, rs):
+def _ensemble(L, T, p, q, runs, t_end, rs, schedule="colours"):
     w = np.zeros(runs)
     for r in range(runs):
         o = Oracle(L, p, q, T, seed=900 + r, threads=2)
+        o.set_schedule(schedule)
         o.init_flat()
         (o.run_rs if rs else o.run)(t_end)
         w[r] = o.measure()[2]
@@ -33,6 +34,16 @@ def test_schedule_bias_vs_true_random_sequential(L, T, p, q, runs, t_end):
     bias = dd - rs
     assert abs(bias) <= 3 * sigma or abs(bias) <= 0.03 * rs, (dd, rs, sigma)
     assert 1.0 < rs < 3.0          # growth really happened (W^2 well above the flat 1/4)
+
+
+def test_dead_border_schedule_bias_vs_true_random_sequential():
+    """Schedule S5 loses 1 - (1-1/T)^2 of the attempts ("impacts the pre-factors of the scaling, but not
+    exponents", P:66): at T = 64 the width after 32 MCS stays within 3 sigma or 5 % of true RS dynamics."""
+    L, T, runs, t_end = 128, 64, 48, 32
+    dd, e1 = _ensemble(L, T, 1.0, 0.0, runs, t_end, rs=False, schedule="dead_border")
+    rs, e2 = _ensemble(L, T, 1.0, 0.0, runs, t_end, rs=True)
+    bias, sigma = dd - rs, np.hypot(e1, e2)
+    assert abs(bias) <= 3 * sigma or abs(bias) <= 0.05 * rs, (dd, rs, sigma)
 
 
 def test_rs_reference_itself_against_exact_L4():
