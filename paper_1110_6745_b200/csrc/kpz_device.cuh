@@ -506,7 +506,10 @@ __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const 
         cur_a[0] = philox4x32_10(0u | ACCEPT, tile_id, P.m, replica, P.key);
         cur_a[1] = philox4x32_10(1u | ACCEPT, tile_id, P.m, replica, P.key);
     }
-#pragma unroll 1
+    // measured on B200 at L = 2^16: 4 calls (32 attempts) per loop body are 4.5 % faster than 1 with the accept
+    // stream off, 2 are best with it on; 16 overflow the instruction cache
+    constexpr int UNROLL = (MODE == 0) ? 4 : 2;
+#pragma unroll UNROLL
     for (uint32_t c = 0; c < CALLS; ++c) {
         // batch c+1 (the last iteration generates one unused batch)
         nxt = philox4x32_10(c + 1u, tile_id, P.m, replica, P.key);
