@@ -1,0 +1,66 @@
+"""Steady-state ensemble harness (BASELINE config 4): R independent replicas of an L x L lattice
+are advanced together by the CUDA library; per-replica W^2 is sampled in the second half of the run and reduced to
+the cumulants kappa_1..kappa_4 (eq. 18), the width distribution Psi_L(x) and the replica-averaged power spectrum S(k)
+(eq. 15-16).  Everything heavy runs in the kernels; this file only drives them and applies analysis.py.
+
+    python -m paper_1110_6745_b200.steady_state --L 128 --replicas 1024 [--t-end N] [--samples 100] [--tile 16]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+
+import numpy as np
+
+from . import analysis
+from .binding import KPZ
+
+
+def run(L, replicas, tile=16, p=1.0, q=0.0, seed=4, t_end=None, samples=100, spectrum_replicas=8, device="cuda:0"):
+    t_end = analysis.steady_state_t_end(L) if t_end is None else int(t_end)
+    k = KPZ(L, p, q, tile, seed, n_replicas=replicas, device=device)
+    try:
+        k.init_flat()
+        t_half = t_end // 2
+        k.run(t_half)
+        step = max(1, (t_end - t_half) // max(1, samples))
+        w2 = []
+        t = t_half
+        while t + step <= t_end:
+            k.run(step)
+            t += step
+            w2.append(k.measure()[2].copy())
+        if t < t_end:
+            k.run(t_end - t)
+        w2 = np.array(w2) if w2 else k.measure()[2][None, :]
+        out = {"L": L, "replicas": replicas, "tile": tile, "p": p, "q": q, "seed": seed, "t_end": t_end,
+               "n_samples": int(w2.size), "cumulants": list(analysis.cumulants(w2)),
+               "W2_final_mean": float(k.measure()[2].mean())}
+        x, psi = analysis.width_distribution(w2)
+        out["psi_x"], out["psi"] = x.tolist(), psi.tolist()
+        if L & (L - 1) == 0 and spectrum_replicas > 0:
+            n = min(replicas, spectrum_replicas)
+            S = np.mean([k.power_spectrum(r)[0] for r in range(n)], axis=0)
+            out["spectrum_replicas"] = n
+            out["S_k"] = S.tolist()
+        return out
+    finally:
+        k.close()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--L", type=int, default=128)
+    ap.add_argument("--replicas", type=int, default=1024)
+    ap.add_argument("--tile", type=int, default=16)
+    ap.add_argument("--p", type=float, default=1.0)
+    ap.add_argument("--q", type=float, default=0.0)
+    ap.add_argument("--seed", type=int, default=4)
+    ap.add_argument("--t-end", type=int, default=None, help="default: 20 L^1.61 (BASELINE config 4)")
+    ap.add_argument("--samples", type=int, default=100)
+    args = ap.parse_args()
+    print(json.dumps(run(args.L, args.replicas, args.tile, args.p, args.q, args.seed, args.t_end, args.samples)))
+
+
+if __name__ == "__main__":
+    main()

@@ -444,3 +444,25 @@ def test_dead_border_replicas_and_full_size_window(pkg):
         assert np.array_equal(gx, osx[M:M + W, M:M + W]) and np.array_equal(gy, osy[M:M + W, M:M + W])
     k.close()
     torch.cuda.empty_cache()
+
+
+def test_steady_state_harness_against_oracle_ensemble(pkg):
+    """The config-4 harness on a small ensemble: its per-sample W^2 values are the oracle's (bit-exact), and the
+    reductions are analysis.py applied to them."""
+    from paper_1110_6745_b200 import steady_state, analysis
+    L, T, R, t_end, samples = 64, 16, 6, 40, 4
+    out = steady_state.run(L, R, tile=T, seed=4, t_end=t_end, samples=samples, spectrum_replicas=2)
+    os_ = [Oracle(L, 1.0, 0.0, T, 4, replica=r, threads=NTHREADS) for r in range(R)]
+    for o in os_:
+        o.init_flat(); o.run(t_end // 2)
+    step = (t_end - t_end // 2) // samples
+    w2 = []
+    for _ in range(samples):
+        for o in os_:
+            o.run(step)
+        w2.append([o.measure()[2] for o in os_])
+    assert out["n_samples"] == R * samples
+    assert out["cumulants"] == list(analysis.cumulants(np.array(w2)))
+    from oracle.spectrum import power_spectrum
+    S = np.mean([power_spectrum(o.heights().astype(np.int64))[0] for o in os_[:2]], axis=0)
+    assert np.allclose(out["S_k"], S, rtol=1e-9, atol=1e-9 * S.max())
