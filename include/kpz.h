@@ -90,6 +90,12 @@ int32_t kpz_run(kpz_ctx* ctx, uint64_t mcs);
 #define KPZ_SCHEDULE_DEAD_BORDER 1
 int32_t kpz_set_schedule(kpz_ctx* ctx, int32_t schedule);
 
+/* Bias-reduction knob (S6): K sub-sweeps per MCS.  Sub-sweep j = 0..K-1 draws its own origin
+ * shift and colour order (global draw with counter word c0 = j) and executes steps [j T^2/K, (j+1) T^2/K) of every
+ * tile's Philox stream; K = 1 (default) is the schedule S4 / S5 itself.  An MCS stays exactly L*L attempts and costs
+ * K times the launches and the tile staging.  K must divide tile*tile/8 (KPZ_EINVAL otherwise). */
+int32_t kpz_set_sub_sweeps(kpz_ctx* ctx, uint32_t K);
+
 /* Height reconstruction (eq. 3) and width (eq. 4).  HOST out-arrays of length n_replicas (any may be NULL).
  * sum_h, sum_h2: exact sums over all sites of h and h^2 with absolute heights anchored by h(0,0) (tracked:
  * 0 at kpz_init_flat, +-2 per accepted flip at site (0,0)).  W2 = (N*sum_h2 - sum_h^2)/N^2, N = L*L, from

@@ -48,6 +48,8 @@ def lib() -> ctypes.CDLL:
         L.kpzo_init_flat.argtypes = [vp]
         L.kpzo_set_schedule.argtypes = [vp, ci]
         L.kpzo_set_schedule.restype = ci
+        L.kpzo_set_sub_sweeps.argtypes = [vp, u32]
+        L.kpzo_set_sub_sweeps.restype = ci
         L.kpzo_run.argtypes = [vp, u64]
         L.kpzo_run.restype = ci
         L.kpzo_run_checked.argtypes = [vp, u64]
@@ -120,6 +122,11 @@ class Oracle:
         """'colours' (S4, default) or 'dead_border' (S5, the paper's own device-level scheme)."""
         if lib().kpzo_set_schedule(self._h, {"colours": 0, "dead_border": 1}[name]) != 0:
             raise ValueError(name)
+
+    def set_sub_sweeps(self, K):
+        """K sub-sweeps per MCS, each with its own origin shift and colour order (S6)."""
+        if lib().kpzo_set_sub_sweeps(self._h, int(K)) != 0:
+            raise ValueError("K must divide T*T")
 
     def init_flat(self):
         lib().kpzo_init_flat(self._h)

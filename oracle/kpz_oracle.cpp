@@ -83,6 +83,7 @@ struct Oracle {
     int64_t h00;
     uint64_t mcs, attempts, deposits, removals;
     int nthreads;
+    uint32_t sub_sweeps;   // K >= 1 sub-sweeps per MCS (S6); K divides T*T
     int schedule;      // 0: four tile colours with halo (S4); 1: dead borders, one pass (S5)
 };
 
@@ -118,8 +119,8 @@ inline int attempt(Oracle* o, uint32_t x, uint32_t y, uint32_t accept_word) {
 }
 
 // global draw of MCS m: offset and colour order.  DESIGN.md "Schedule" S2.
-void global_draw(const Oracle* o, uint32_t m, uint32_t* ox, uint32_t* oy, uint32_t perm[4]) {
-    uint32_t ctr[4] = {0u, 0xFFFFFFFFu, m, o->replica};
+void global_draw(const Oracle* o, uint32_t m, uint32_t sub, uint32_t* ox, uint32_t* oy, uint32_t perm[4]) {
+    uint32_t ctr[4] = {sub, 0xFFFFFFFFu, m, o->replica};   // S6: sub-sweep j of MCS m draws with c0 = j (j = 0: S2)
     uint32_t key[2] = {(uint32_t)(o->seed & 0xFFFFFFFFu), (uint32_t)(o->seed >> 32)};
     uint32_t G[4];
     philox4x32_10(ctr, key, G);
@@ -140,7 +141,7 @@ void global_draw(const Oracle* o, uint32_t m, uint32_t* ox, uint32_t* oy, uint32
 
 // all T*T sequential steps of tile (tx,ty) in MCS m.  DESIGN.md "Schedule" S3.
 void run_tile(Oracle* o, uint32_t m, uint32_t ox, uint32_t oy, uint32_t tx, uint32_t ty,
-              uint64_t* n_dep, uint64_t* n_rem, int64_t* dh00) {
+              uint64_t* n_dep, uint64_t* n_rem, int64_t* dh00, uint32_t s_begin, uint32_t s_end) {
     const uint32_t T = o->T, L = o->L;
     const uint32_t tile_id = ty * o->NT + tx;
     const uint32_t key[2] = {(uint32_t)(o->seed & 0xFFFFFFFFu), (uint32_t)(o->seed >> 32)};
@@ -150,12 +151,12 @@ void run_tile(Oracle* o, uint32_t m, uint32_t ox, uint32_t oy, uint32_t tx, uint
     // step s takes digit s & 1 of word (s >> 1) & 3 of call R(s >> 3, ...); its accept word is word s & 3 of call
     // R((s >> 2) | 0x80000000, ...).
     uint32_t QS[4] = {0, 0, 0, 0}, QA[4] = {0, 0, 0, 0};
-    for (uint32_t s = 0; s < steps; ++s) {
-        if ((s & 7u) == 0u) {
+    for (uint32_t s = s_begin; s < s_end; ++s) {
+        if ((s & 7u) == 0u || s == s_begin) {
             uint32_t ctr_s[4] = {s >> 3, tile_id, m, o->replica};
             philox4x32_10(ctr_s, key, QS);
         }
-        if ((s & 3u) == 0u) {
+        if ((s & 3u) == 0u || s == s_begin) {
             uint32_t ctr_a[4] = {(s >> 2) | 0x80000000u, tile_id, m, o->replica};
             philox4x32_10(ctr_a, key, QA);
         }
@@ -187,10 +188,10 @@ bool tile_touches_window(const Oracle* o, uint32_t ox, uint32_t oy, uint32_t tx,
     return hitx && hity;
 }
 
-void run_one_mcs(Oracle* o) {
-    const uint32_t m = (uint32_t)o->mcs;
+// one sub-sweep: steps [s_begin, s_end) of every tile's stream of MCS m, in the frame and colour order of draw `sub`
+void run_sub_sweep(Oracle* o, uint32_t m, uint32_t sub, uint32_t s_begin, uint32_t s_end) {
     uint32_t ox, oy, perm[4];
-    global_draw(o, m, &ox, &oy, perm);
+    global_draw(o, m, sub, &ox, &oy, perm);
     const uint32_t NT = o->NT;
     if (o->schedule == 1) {
         // S5: every tile in one pass; the tiles are independent because their edge sites are dead
@@ -200,12 +201,10 @@ void run_one_mcs(Oracle* o) {
         for (int64_t ty = 0; ty < (int64_t)NT; ++ty) {
             for (int64_t tx = 0; tx < (int64_t)NT; ++tx) {
                 if (!tile_touches_window(o, ox, oy, (uint32_t)tx, (uint32_t)ty)) continue;
-                run_tile(o, m, ox, oy, (uint32_t)tx, (uint32_t)ty, &n_dep, &n_rem, &dh00);
+                run_tile(o, m, ox, oy, (uint32_t)tx, (uint32_t)ty, &n_dep, &n_rem, &dh00, s_begin, s_end);
             }
         }
         o->deposits += n_dep; o->removals += n_rem; o->h00 += dh00;
-        o->attempts += (uint64_t)o->L * o->L;
-        o->mcs += 1;
         return;
     }
     for (int i = 0; i < 4; ++i) {
@@ -219,11 +218,18 @@ void run_one_mcs(Oracle* o) {
             for (int64_t k = 0; k < half; ++k) {
                 uint32_t ty = (uint32_t)(2 * j) + cy, tx = (uint32_t)(2 * k) + cx;
                 if (!tile_touches_window(o, ox, oy, tx, ty)) continue;
-                run_tile(o, m, ox, oy, tx, ty, &n_dep, &n_rem, &dh00);
+                run_tile(o, m, ox, oy, tx, ty, &n_dep, &n_rem, &dh00, s_begin, s_end);
             }
         }
         o->deposits += n_dep; o->removals += n_rem; o->h00 += dh00;
     }
+}
+
+// S4 / S5 / S6: one MCS = K sub-sweeps, sub-sweep j executing steps [j T^2/K, (j+1) T^2/K) of every tile
+void run_one_mcs(Oracle* o) {
+    const uint32_t m = (uint32_t)o->mcs;
+    const uint32_t steps = o->T * o->T, K = o->sub_sweeps;
+    for (uint32_t j = 0; j < K; ++j) run_sub_sweep(o, m, j, j * (steps / K), (j + 1) * (steps / K));
     o->attempts += (uint64_t)o->L * o->L;
     o->mcs += 1;
 }
@@ -288,6 +294,7 @@ void* kpzo_create(uint32_t L, double p, double q, uint32_t T, uint64_t seed, uin
     o->seed = seed; o->replica = replica; o->p = p; o->q = q;
     o->thr_p = threshold(p); o->thr_q = threshold(q);
     o->schedule = 0;
+    o->sub_sweeps = 1;
     o->full = (ww == 0 && wh == 0);
     if (o->full) { wx0 = wy0 = 0; ww = wh = L; }
     if (ww > L || wh > L) { delete o; return nullptr; }
@@ -333,6 +340,14 @@ int kpzo_set_schedule(void* h, int schedule) {
     return 0;
 }
 
+// K sub-sweeps per MCS (S6); K >= 1 must divide T*T.  Returns 0 or -1.
+int kpzo_set_sub_sweeps(void* h, uint32_t K) {
+    Oracle* o = static_cast<Oracle*>(h);
+    if (K < 1 || (o->T * o->T) % K != 0) return -1;
+    o->sub_sweeps = K;
+    return 0;
+}
+
 int kpzo_run(void* h, uint64_t n_mcs) {
     Oracle* o = (Oracle*)h;
     for (uint64_t i = 0; i < n_mcs; ++i) {
@@ -357,7 +372,7 @@ int kpzo_run_checked(void* h, uint64_t n_mcs) {
     for (uint64_t it = 0; it < n_mcs; ++it) {
         const uint32_t m = (uint32_t)o->mcs;
         uint32_t ox, oy, perm[4];
-        global_draw(o, m, &ox, &oy, perm);
+        global_draw(o, m, 0u, &ox, &oy, perm);
         for (int i = 0; i < 4; ++i) {
             uint32_t cx = perm[i] & 1u, cy = perm[i] >> 1;
             for (uint32_t ty = cy; ty < o->NT; ty += 2)
@@ -462,7 +477,7 @@ void kpzo_counters(void* h, uint64_t* attempts, uint64_t* deposits, uint64_t* re
 }
 
 void kpzo_global_draw(void* h, uint32_t m, uint32_t* ox, uint32_t* oy, uint32_t* perm) {
-    global_draw((Oracle*)h, m, ox, oy, perm);
+    global_draw((Oracle*)h, m, 0u, ox, oy, perm);
 }
 
 // True single-site random-sequential reference dynamics (NOT the schedule; used only to bound the bias of the

@@ -43,9 +43,10 @@ def threshold(prob):
 
 
 class Twin:
-    def __init__(self, L, p, q, T, seed, replica=0, schedule="colours"):
+    def __init__(self, L, p, q, T, seed, replica=0, schedule="colours", sub_sweeps=1):
         assert T >= 1 and L % (2 * T) == 0 and schedule in ("colours", "dead_border")
-        self.schedule = schedule
+        assert sub_sweeps >= 1 and (T * T) % sub_sweeps == 0
+        self.schedule, self.K = schedule, sub_sweeps
         self.L, self.T, self.p, self.q, self.seed, self.replica = L, T, p, q, seed, replica
         self.g = 4 if T % 4 == 0 else 1
         self.key = (seed & MASK, (seed >> 32) & MASK)
@@ -81,8 +82,8 @@ class Twin:
         if self.trace is not None:
             self.trace.append((x, y, d))
 
-    def global_draw(self, m):
-        G = philox4x32_10((0, MASK, m, self.replica), self.key)
+    def global_draw(self, m, sub=0):
+        G = philox4x32_10((sub, MASK, m, self.replica), self.key)
         n = self.T // self.g
         ox = self.g * mulhi32(G[0], n)
         oy = self.g * mulhi32(G[1], n)
@@ -97,20 +98,23 @@ class Twin:
         NT = L // T
         for _ in range(n_mcs):
             m = self.mcs
-            ox, oy, perm = self.global_draw(m)
-            # S4: the four colours in the drawn order; S5 (dead borders): every tile in one pass
-            passes = [[(tx, ty) for ty in range(c >> 1, NT, 2) for tx in range(c & 1, NT, 2)] for c in perm] \
-                if self.schedule == "colours" else [[(tx, ty) for ty in range(NT) for tx in range(NT)]]
-            for tiles in passes:
-                for (tx, ty) in tiles:
-                    if True:
+            # S6: K sub-sweeps; sub-sweep j has its own draw (offset, colour order) and runs steps
+            # [j T^2/K, (j+1) T^2/K) of every tile's stream of this MCS
+            for j in range(self.K):
+                ox, oy, perm = self.global_draw(m, j)
+                # S4: the four colours in the drawn order; S5 (dead borders): every tile in one pass
+                passes = [[(tx, ty) for ty in range(c >> 1, NT, 2) for tx in range(c & 1, NT, 2)] for c in perm] \
+                    if self.schedule == "colours" else [[(tx, ty) for ty in range(NT) for tx in range(NT)]]
+                for tiles in passes:
+                    for (tx, ty) in tiles:
                         tile_id = ty * NT + tx
-                        for s in range(T * T):
+                        s0 = j * T * T // self.K
+                        for s in range(s0, (j + 1) * T * T // self.K):
                             # DESIGN.md S3: a site word is a base-T*T fraction with two digits; step s uses digit
                             # s % 2 of word (s // 2) % 4 of call s // 8; accept word = word s % 4 of call s // 4 + 2^31
-                            if s % 8 == 0:
+                            if s % 8 == 0 or s == s0:
                                 sites = philox4x32_10((s // 8, tile_id, m, self.replica), self.key)
-                            if s % 4 == 0:
+                            if s % 4 == 0 or s == s0:
                                 accepts = philox4x32_10((s // 4 + 0x80000000, tile_id, m, self.replica), self.key)
                             word = sites[(s // 2) % 4]
                             if s % 2 == 1:

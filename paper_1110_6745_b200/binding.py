@@ -21,7 +21,7 @@ exported_symbols = [
     "kpz_workspace_bytes", "kpz_create", "kpz_create_batch", "kpz_bind", "kpz_init_flat", "kpz_run", "kpz_measure",
     "kpz_destroy", "kpz_synchronize", "kpz_last_error", "kpz_get_slopes", "kpz_get_window", "kpz_set_slopes",
     "kpz_state_hash", "kpz_counters", "kpz_export_packed", "kpz_import_packed", "kpz_step_host",
-    "kpz_launch_count", "kpz_philox_selftest", "kpz_profiles", "kpz_power_spectrum", "kpz_set_schedule",
+    "kpz_launch_count", "kpz_philox_selftest", "kpz_profiles", "kpz_power_spectrum", "kpz_set_schedule", "kpz_set_sub_sweeps",
 ]
 
 
@@ -58,6 +58,7 @@ def load_library() -> ctypes.CDLL:
         "kpz_state_hash": [vp, u32, vp],
         "kpz_counters": [vp, u32, vp, vp, vp, vp, vp],
         "kpz_set_schedule": [vp, i32],
+        "kpz_set_sub_sweeps": [vp, u32],
         "kpz_profiles": [vp, u32, vp, vp],
         "kpz_power_spectrum": [vp, u32, vp, vp, vp],
         "kpz_export_packed": [vp, vp, sz],
@@ -169,6 +170,10 @@ class KPZ:
     def set_schedule(self, name):
         """kpz_set_schedule: 'colours' (default) or 'dead_border' (the paper's own scheme)."""
         self._check(self._lib.kpz_set_schedule(self._h, {"colours": 0, "dead_border": 1}[name]))
+
+    def set_sub_sweeps(self, K):
+        """kpz_set_sub_sweeps: K sub-sweeps per MCS, each with its own origin shift and colour order."""
+        self._check(self._lib.kpz_set_sub_sweeps(self._h, int(K)))
 
     def profiles(self, replica=0):
         """kpz_profiles: exact (col_sums[x] = sum_y h, row_sums[y] = sum_x h), int64 arrays of length L."""

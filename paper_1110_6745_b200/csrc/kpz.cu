@@ -91,6 +91,7 @@ struct kpz_ctx {
     uint64_t mcs;            // completed MCS (all replicas advance together)
     uint64_t launches;
     int32_t schedule;        // KPZ_SCHEDULE_COLOURS or KPZ_SCHEDULE_DEAD_BORDER
+    uint32_t sub_sweeps;     // K sub-sweeps per MCS (S6)
     uint32_t* d_lattice;
     unsigned char* d_scratch;
     cudaStream_t stream;
@@ -127,10 +128,10 @@ int grid_for(uint64_t n, int block, int cap = 148 * 16) {
     return (int)g;
 }
 
-template <int T, int NTHR, int MODE, bool DEAD>
-int32_t launch_update_t(kpz_ctx* c, const kpz::UpdateParams& P) {
+template <int T, int NTHR, int MODE, bool DEAD, bool SUB>
+int32_t launch_update_k(kpz_ctx* c, const kpz::UpdateParams& P) {
     const size_t smem = (size_t)kpz::TileGeom<T>::WORDS * NTHR * sizeof(uint32_t);
-    auto kern = kpz::kpz_update_kernel<T, NTHR, MODE, DEAD>;
+    auto kern = kpz::kpz_update_kernel<T, NTHR, MODE, DEAD, SUB>;
     static bool attr_set = false;
     if (!attr_set) {
         KPZ_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -143,6 +144,11 @@ int32_t launch_update_t(kpz_ctx* c, const kpz::UpdateParams& P) {
     KPZ_CUDA(c, cudaGetLastError());
     c->launches++;
     return KPZ_OK;
+}
+
+template <int T, int NTHR, int MODE, bool DEAD>
+int32_t launch_update_t(kpz_ctx* c, const kpz::UpdateParams& P) {
+    return c->sub_sweeps > 1 ? launch_update_k<T, NTHR, MODE, DEAD, true>(c, P) : launch_update_k<T, NTHR, MODE, DEAD, false>(c, P);
 }
 
 template <int T, int NTHR, bool DEAD>
@@ -158,7 +164,7 @@ int32_t launch_update_mode(kpz_ctx* c, const kpz::UpdateParams& P) {
                                                    : launch_update_sched<T, NTHR, false>(c, P);
 }
 
-int32_t launch_update(kpz_ctx* c, uint32_t m, uint32_t slot) {
+int32_t launch_update(kpz_ctx* c, uint32_t m, uint32_t slot, uint32_t sub) {
     kpz::UpdateParams P;
     P.lattice = c->d_lattice;
     P.stats = reinterpret_cast<unsigned long long*>(c->d_scratch + c->sl.stats);
@@ -176,6 +182,10 @@ int32_t launch_update(kpz_ctx* c, uint32_t m, uint32_t slot) {
     P.tq_incl = (uint32_t)(P.thr_q - 1);
     P.m = m;
     P.slot = slot;
+    P.sub = sub;
+    const uint32_t calls = c->T * c->T / 8u, per = calls / c->sub_sweeps;
+    P.call_begin = sub * per;
+    P.call_end = (sub + 1u) * per;
     P.key.k0 = (uint32_t)(c->seed & 0xFFFFFFFFull);
     P.key.k1 = (uint32_t)(c->seed >> 32);
     switch (c->T) {
@@ -259,7 +269,7 @@ int32_t kpz_create_batch(kpz_ctx** out, uint32_t L, double p, double q, uint32_t
     kpz_ctx* c = new (std::nothrow) kpz_ctx();
     if (!c) return KPZ_ENOMEM;
     c->L = L; c->T = tile; c->R = n_replicas; c->p = p; c->q = q; c->seed = seed;
-    c->mcs = 0; c->launches = 0; c->schedule = KPZ_SCHEDULE_COLOURS;
+    c->mcs = 0; c->launches = 0; c->schedule = KPZ_SCHEDULE_COLOURS; c->sub_sweeps = 1;
     c->d_lattice = nullptr; c->d_scratch = nullptr; c->stream = nullptr; c->bound = false;
     c->sl = scratch_layout(L, n_replicas);
     c->lattice_bytes = (size_t)n_replicas * ((size_t)L * L / 4);
@@ -306,9 +316,11 @@ int32_t kpz_run(kpz_ctx* c, uint64_t mcs) {
     for (uint64_t k = 0; k < mcs; ++k) {
         const uint32_t m = (uint32_t)c->mcs;
         const uint32_t passes = (c->schedule == KPZ_SCHEDULE_DEAD_BORDER) ? 1u : 4u;
-        for (uint32_t slot = 0; slot < passes; ++slot) {
-            rc = launch_update(c, m, slot);
-            if (rc != KPZ_OK) return rc;
+        for (uint32_t sub = 0; sub < c->sub_sweeps; ++sub) {
+            for (uint32_t slot = 0; slot < passes; ++slot) {
+                rc = launch_update(c, m, slot, sub);
+                if (rc != KPZ_OK) return rc;
+            }
         }
         c->mcs++;
     }
@@ -319,6 +331,14 @@ int32_t kpz_set_schedule(kpz_ctx* c, int32_t schedule) {
     if (!c) return KPZ_EINVAL;
     if (schedule != KPZ_SCHEDULE_COLOURS && schedule != KPZ_SCHEDULE_DEAD_BORDER) return fail(c, KPZ_EINVAL, "unknown schedule");
     c->schedule = schedule;
+    return KPZ_OK;
+}
+
+int32_t kpz_set_sub_sweeps(kpz_ctx* c, uint32_t K) {
+    if (!c) return KPZ_EINVAL;
+    const uint32_t calls = c->T * c->T / 8u;
+    if (K < 1 || K > calls || calls % K != 0) return fail(c, KPZ_EINVAL, "sub-sweeps must divide tile*tile/8");
+    c->sub_sweeps = K;
     return KPZ_OK;
 }
 

@@ -67,15 +67,17 @@ struct UpdateParams {
     uint32_t blocked;              // 1: 8x4 lane blocking of tiles (HN % 8 == 0), 0: linear
     uint32_t m;                    // MCS index (number of completed MCS)
     uint32_t slot;                 // 0..3: which entry of the colour order this launch executes
+    uint32_t sub;                  // sub-sweep index j (S6): counter word c0 of the global draw
+    uint32_t call_begin, call_end; // site calls [call_begin, call_end) of every tile: steps 8*call_begin .. 8*call_end
     PhiloxKey key;
 };
 
 // Global draw of MCS m for one replica: offset (multiples of 4 sites) and colour order.
 // DESIGN.md "Schedule" S2.  Returns the colour processed in `slot`.
 template <int T>
-__device__ __forceinline__ void global_draw(const UpdateParams& P, uint32_t replica, uint32_t& ox, uint32_t& oy,
+__device__ __forceinline__ void global_draw(const UpdateParams& P, uint32_t sub, uint32_t replica, uint32_t& ox, uint32_t& oy,
                                             uint32_t& colour) {
-    const uint4 G = philox4x32_10(0u, 0xFFFFFFFFu, P.m, replica, P.key);
+    const uint4 G = philox4x32_10(sub, 0xFFFFFFFFu, P.m, replica, P.key);
     constexpr uint32_t g = 4;
     ox = g * mulhi32(G.x, T / g);
     oy = g * mulhi32(G.y, T / g);
@@ -493,24 +495,25 @@ __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site
 // evaluated only in MODE 1.  Calls are generated one batch ahead of the attempts that consume them (the generator
 // is counter-based, so the next batch does not depend on the lattice): the multiplier pipe works on batch b+1
 // while the shared-memory round trips of batch b are in flight.
-template <int T, int NTHR, int MODE, bool TRACK, bool DEAD>
+template <int T, int NTHR, int MODE, bool TRACK, bool DEAD, bool WHOLE>
 __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const UpdateParams& P, uint32_t tile_id,
                                                uint32_t replica, uint32_t& n_dep, uint32_t& n_rem, int32_t& dh00,
                                                uint32_t origin_idx) {
-    constexpr uint32_t CALLS = (uint32_t)(T * T) / 8u;
     constexpr uint32_t ACCEPT = 0x80000000u;
     constexpr uint32_t TT = (uint32_t)(T * T);
+    // WHOLE: all T*T/8 site calls of the tile (compile-time trip count); otherwise one sub-sweep's slice (S6)
+    const uint32_t c_begin = WHOLE ? 0u : P.call_begin, c_end = WHOLE ? (uint32_t)(T * T) / 8u : P.call_end;
     uint4 cur, nxt, cur_a[2], nxt_a[2];
-    cur = philox4x32_10(0u, tile_id, P.m, replica, P.key);
+    cur = philox4x32_10(c_begin, tile_id, P.m, replica, P.key);
     if (MODE) {
-        cur_a[0] = philox4x32_10(0u | ACCEPT, tile_id, P.m, replica, P.key);
-        cur_a[1] = philox4x32_10(1u | ACCEPT, tile_id, P.m, replica, P.key);
+        cur_a[0] = philox4x32_10((2u * c_begin) | ACCEPT, tile_id, P.m, replica, P.key);
+        cur_a[1] = philox4x32_10((2u * c_begin + 1u) | ACCEPT, tile_id, P.m, replica, P.key);
     }
     // measured on B200 at L = 2^16: 4 calls (32 attempts) per loop body are 4.5 % faster than 1 with the accept
     // stream off, 2 are best with it on; 16 overflow the instruction cache
     constexpr int UNROLL = (MODE == 0) ? 4 : 2;
 #pragma unroll UNROLL
-    for (uint32_t c = 0; c < CALLS; ++c) {
+    for (uint32_t c = c_begin; c < c_end; ++c) {
         // batch c+1 (the last iteration generates one unused batch)
         nxt = philox4x32_10(c + 1u, tile_id, P.m, replica, P.key);
         if (MODE) {
@@ -537,7 +540,8 @@ __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const 
 
 // DEAD = false: one colour of schedule S4 per launch (P.slot);  DEAD = true: every tile of the dead-border schedule
 // S5 in one launch (P.HN = NT).
-template <int T, int NTHR, int MODE, bool DEAD>
+// SUB = true: one sub-sweep (S6), site calls [P.call_begin, P.call_end) of every tile instead of all of them.
+template <int T, int NTHR, int MODE, bool DEAD, bool SUB>
 __global__ void __launch_bounds__(NTHR) kpz_update_kernel(const UpdateParams P) {
     using G = TileGeom<T>;
     extern __shared__ uint32_t smem[];
@@ -561,7 +565,7 @@ __global__ void __launch_bounds__(NTHR) kpz_update_kernel(const UpdateParams P) 
         }
     }
     uint32_t ox, oy, colour;
-    global_draw<T>(P, replica, ox, oy, colour);
+    global_draw<T>(P, SUB ? P.sub : 0u, replica, ox, oy, colour);
     const uint32_t tx = DEAD ? i : 2u * i + (colour & 1u), ty = DEAD ? j : 2u * j + (colour >> 1);
     const uint32_t X0 = ox + tx * T, Y0 = oy + ty * T;        // < L + T
     const uint32_t tile_id = ty * P.NT + tx;
@@ -587,9 +591,9 @@ __global__ void __launch_bounds__(NTHR) kpz_update_kernel(const UpdateParams P) 
     if (active) {
         // ---- a3 + a4: T*T sequential attempts ----
         if (any_origin)
-            run_tile_steps<T, NTHR, MODE, true, DEAD>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx);
+            run_tile_steps<T, NTHR, MODE, true, DEAD, !SUB>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx);
         else
-            run_tile_steps<T, NTHR, MODE, false, DEAD>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx);
+            run_tile_steps<T, NTHR, MODE, false, DEAD, !SUB>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx);
         // ---- a5: write back ----
         if constexpr (G::WIDE) stage_out_wide<T, NTHR, StageBatch<T>::N, DEAD>(planeX, planeY, L, W, x0, y0, sm);
         else stage_out_narrow<T, NTHR, DEAD>(planeX, planeY, L, W, x0, y0, sm);

@@ -466,3 +466,26 @@ def test_steady_state_harness_against_oracle_ensemble(pkg):
     from oracle.spectrum import power_spectrum
     S = np.mean([power_spectrum(o.heights().astype(np.int64))[0] for o in os_[:2]], axis=0)
     assert np.allclose(out["S_k"], S, rtol=1e-9, atol=1e-9 * S.max())
+
+
+@pytest.mark.parametrize("L,T,p,q,K,sched,seed", [
+    (64, 8, 1.0, 0.0, 2, "colours", 41),
+    (96, 16, 0.75, 0.25, 8, "colours", 42),
+    (128, 32, 1.0, 0.0, 4, "dead_border", 43),
+    (512, 64, 1.0, 0.0, 16, "colours", 44),
+    (512, 64, 0.6, 0.2, 512, "colours", 45),       # one site call per tile and sub-sweep
+])
+def test_sub_sweeps_parity(pkg, L, T, p, q, K, sched, seed):
+    """Schedule S6 (bias-reduction knob): K sub-sweeps per MCS; bit-exact state, sums, counters."""
+    k = pkg.KPZ(L, p, q, T, seed)
+    k.set_schedule(sched); k.set_sub_sweeps(K)
+    k.init_flat()
+    o = Oracle(L, p, q, T, seed, threads=NTHREADS)
+    o.set_schedule(sched); o.set_sub_sweeps(K)
+    o.init_flat()
+    for t in range(3):
+        k.run(1); o.run(1)
+        _compare_full(k, o)
+        _compare_scalars(k, [o])
+    with pytest.raises(pkg.KpzError):
+        k.set_sub_sweeps(3)

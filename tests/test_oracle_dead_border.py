@@ -63,3 +63,28 @@ def test_lost_attempts_fraction_and_thread_independence():
     ratio = res[0][2] / c.counters()["deposits"]
     assert live - 0.05 < ratio < 1.0
     assert c.counters()["attempts"] == 3 * L * L == Oracle.counters(o)["attempts"]
+
+
+@pytest.mark.parametrize("L,T,p,q,K,sched", [(16, 4, 1.0, 0.0, 2, "colours"), (24, 3, 0.6, 0.3, 3, "colours"),
+                                             (32, 8, 0.75, 0.25, 8, "dead_border"), (32, 4, 1.0, 0.0, 16, "colours")])
+def test_sub_sweeps_oracle_equals_twin(L, T, p, q, K, sched):
+    """Schedule S6: K sub-sweeps per MCS, each with its own draw, over consecutive slices of the tile streams."""
+    o = Oracle(L, p, q, T, 5)
+    o.set_schedule(sched); o.set_sub_sweeps(K)
+    o.init_flat(); o.run(3)
+    t = kpz_twin.Twin(L, p, q, T, 5, schedule=sched, sub_sweeps=K)
+    t.init_flat(); t.run(3)
+    sx, sy = o.slopes()
+    tx, ty = t.slopes()
+    assert np.array_equal(sx, np.array(tx)) and np.array_equal(sy, np.array(ty))
+    assert o.measure()[:2] == t.sums() and o.check() == 0
+    assert o.counters()["attempts"] == 3 * L * L
+
+
+def test_sub_sweeps_one_is_the_default_and_bad_values_are_rejected():
+    a = Oracle(64, 1.0, 0.0, 16, 9); a.init_flat(); a.run(2)
+    b = Oracle(64, 1.0, 0.0, 16, 9); b.set_sub_sweeps(1); b.init_flat(); b.run(2)
+    c = Oracle(64, 1.0, 0.0, 16, 9); c.set_sub_sweeps(4); c.init_flat(); c.run(2)
+    assert a.state_hash() == b.state_hash() != c.state_hash()
+    with pytest.raises(ValueError):
+        a.set_sub_sweeps(7)
