@@ -542,7 +542,9 @@ __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const 
 // S5 in one launch (P.HN = NT).
 // SUB = true: one sub-sweep (S6), site calls [P.call_begin, P.call_end) of every tile instead of all of them.
 template <int T, int NTHR, int MODE, bool DEAD, bool SUB>
-__global__ void __launch_bounds__(NTHR) kpz_update_kernel(const UpdateParams P) {
+// T = 64: 8 CTAs fit the shared memory; asking for 10 caps the registers at 204, which measured best on B200
+// (168, ptxas' own choice: -1.5 %; 255: -1.5 %)
+__global__ void __launch_bounds__(NTHR, (T == 64) ? 10 : 1) kpz_update_kernel(const UpdateParams P) {
     using G = TileGeom<T>;
     extern __shared__ uint32_t smem[];
     uint32_t* sm = smem + threadIdx.x;
