@@ -103,6 +103,14 @@ int32_t kpz_set_sub_sweeps(kpz_ctx* ctx, uint32_t K);
  * Does not modify the lattice.  KPZ_EOVERFLOW if a requested sum does not fit int64 (W2 is still written). */
 int32_t kpz_measure(kpz_ctx* ctx, int64_t* sum_h, int64_t* sum_h2, double* W2);
 
+/* Sampling-time driver ("the program calculates and writes out the width" at the times t_i of eq. 8):
+ * advances to each absolute MCS clock times[i] (HOST array, strictly increasing, times[0] >= the current clock)
+ * and measures there.  HOST out-arrays of n_times * n_replicas entries, sample-major [i * n_replicas + r] (any may
+ * be NULL).  Equivalent to the kpz_run / kpz_measure calls it makes; returns KPZ_EOVERFLOW if any sample's int64
+ * sum overflowed (W2 still written), KPZ_EINVAL for a bad time list. */
+int32_t kpz_run_sampled(kpz_ctx* ctx, const uint64_t* times, uint32_t n_times, int64_t* sum_h, int64_t* sum_h2,
+                        double* W2);
+
 /* Frees the handle (not the bound buffers).  NULL is a no-op. */
 int32_t kpz_destroy(kpz_ctx* ctx);
 

@@ -21,7 +21,7 @@ exported_symbols = [
     "kpz_workspace_bytes", "kpz_create", "kpz_create_batch", "kpz_bind", "kpz_init_flat", "kpz_run", "kpz_measure",
     "kpz_destroy", "kpz_synchronize", "kpz_last_error", "kpz_get_slopes", "kpz_get_window", "kpz_set_slopes",
     "kpz_state_hash", "kpz_counters", "kpz_export_packed", "kpz_import_packed", "kpz_step_host",
-    "kpz_launch_count", "kpz_philox_selftest", "kpz_profiles", "kpz_power_spectrum", "kpz_set_schedule", "kpz_set_sub_sweeps",
+    "kpz_launch_count", "kpz_philox_selftest", "kpz_profiles", "kpz_power_spectrum", "kpz_set_schedule", "kpz_set_sub_sweeps", "kpz_run_sampled",
 ]
 
 
@@ -57,6 +57,7 @@ def load_library() -> ctypes.CDLL:
         "kpz_set_slopes": [vp, u32, vp, vp, i64],
         "kpz_state_hash": [vp, u32, vp],
         "kpz_counters": [vp, u32, vp, vp, vp, vp, vp],
+        "kpz_run_sampled": [vp, vp, u32, vp, vp, vp],
         "kpz_set_schedule": [vp, i32],
         "kpz_set_sub_sweeps": [vp, u32],
         "kpz_profiles": [vp, u32, vp, vp],
@@ -166,6 +167,17 @@ class KPZ:
         if sx.shape != (self.L, self.L) or sy.shape != (self.L, self.L):
             raise ValueError("slope arrays must be L x L")
         self._check(self._lib.kpz_set_slopes(self._h, replica, sx.ctypes.data, sy.ctypes.data, int(h00)))
+
+    def run_sampled(self, times):
+        """kpz_run_sampled: (sum_h, sum_h2, W2) arrays of shape [len(times), n_replicas] at the absolute MCS clocks."""
+        t = np.ascontiguousarray(times, dtype=np.uint64)
+        n = len(t)
+        s1 = np.zeros((n, self.n_replicas), dtype=np.int64)
+        s2 = np.zeros((n, self.n_replicas), dtype=np.int64)
+        w2 = np.zeros((n, self.n_replicas), dtype=np.float64)
+        self._check(self._lib.kpz_run_sampled(self._h, t.ctypes.data, n, s1.ctypes.data, s2.ctypes.data, w2.ctypes.data),
+                    allow=(KPZ_EOVERFLOW,))
+        return s1, s2, w2
 
     def set_schedule(self, name):
         """kpz_set_schedule: 'colours' (default) or 'dead_border' (the paper's own scheme)."""

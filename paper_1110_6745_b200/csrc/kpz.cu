@@ -366,6 +366,27 @@ int32_t kpz_measure(kpz_ctx* c, int64_t* sum_h, int64_t* sum_h2, double* W2) {
     return KPZ_OK;
 }
 
+int32_t kpz_run_sampled(kpz_ctx* c, const uint64_t* times, uint32_t n_times, int64_t* sum_h, int64_t* sum_h2, double* W2) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    if (!times || n_times == 0) return fail(c, KPZ_EINVAL, "no sampling times");
+    uint64_t prev = c->mcs;
+    for (uint32_t i = 0; i < n_times; ++i) {
+        if (times[i] < prev || (i > 0 && times[i] == times[i - 1])) return fail(c, KPZ_EINVAL, "sampling times must increase from the current MCS clock");
+        prev = times[i];
+    }
+    int32_t worst = KPZ_OK;
+    for (uint32_t i = 0; i < n_times; ++i) {
+        rc = kpz_run(c, times[i] - c->mcs);
+        if (rc != KPZ_OK) return rc;
+        const size_t o = (size_t)i * c->R;
+        rc = kpz_measure(c, sum_h ? sum_h + o : nullptr, sum_h2 ? sum_h2 + o : nullptr, W2 ? W2 + o : nullptr);
+        if (rc == KPZ_EOVERFLOW) worst = rc;
+        else if (rc != KPZ_OK) return rc;
+    }
+    return worst;
+}
+
 int32_t kpz_destroy(kpz_ctx* c) {
     delete c;
     return KPZ_OK;

@@ -489,3 +489,25 @@ def test_sub_sweeps_parity(pkg, L, T, p, q, K, sched, seed):
         _compare_scalars(k, [o])
     with pytest.raises(pkg.KpzError):
         k.set_sub_sweeps(3)
+
+
+def test_run_sampled_config1_times(pkg):
+    """kpz_run_sampled on BASELINE config 1 (L=256, T=16, p=1, q=0, seed 1; t = 1,2,4,...,64): every sample equals the
+    oracle's, and the call equals the run/measure sequence it stands for."""
+    L, T, seed = 256, 16, 1
+    times = [1, 2, 4, 8, 16, 32, 64]
+    k = pkg.KPZ(L, 1.0, 0.0, T, seed)
+    k.init_flat()
+    s1, s2, w2 = k.run_sampled(times)
+    o = Oracle(L, 1.0, 0.0, T, seed, threads=NTHREADS)
+    o.init_flat()
+    done = 0
+    for i, t in enumerate(times):
+        o.run(t - done); done = t
+        os1, os2, ow2 = o.measure()
+        assert (int(s1[i, 0]), int(s2[i, 0]), float(w2[i, 0])) == (os1, os2, ow2)
+    assert k.counters()["mcs"] == 64 and k.state_hash() == o.state_hash()
+    with pytest.raises(pkg.KpzError):
+        k.run_sampled([10, 20])            # behind the MCS clock
+    with pytest.raises(pkg.KpzError):
+        k.run_sampled([70, 70])
