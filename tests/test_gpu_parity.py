@@ -189,8 +189,8 @@ CONFIG2_TIMES = [1, 2, 3, 4, 5, 7, 9, 11, 14, 17, 22, 28, 36, 45, 57, 73, 92, 11
 
 def test_config2_prefix(pkg):
     """BASELINE config 2: L=4096, T=32, p=1, q=0, seed 7; the log-spaced sample times up to KPZ_CONFIG2_TMAX
-    (default 45; 1000 = the whole config) with the full state compared at every sample."""
-    tmax = int(os.environ.get("KPZ_CONFIG2_TMAX", "45"))
+    (default 1000 = the whole config, 27 samples, about 50 s of oracle time) with the full state compared at every sample."""
+    tmax = int(os.environ.get("KPZ_CONFIG2_TMAX", "1000"))
     L, T, seed = 4096, 32, 7
     k = pkg.KPZ(L, 1.0, 0.0, T, seed)
     k.init_flat()
@@ -276,7 +276,7 @@ def test_config3_full_size_windows_and_invariants(pkg):
     times: sampled windows vs the light-cone window oracle + properties that hold at any size."""
     import torch
     torch.cuda.empty_cache()
-    L, T, seed, n = 1 << 17, 64, 42, 2
+    L, T, seed, n = 1 << 17, 64, 42, 4
     k = pkg.KPZ(L, 1.0, 0.0, T, seed)
     k.init_flat()
     k.run(n)
@@ -284,7 +284,7 @@ def test_config3_full_size_windows_and_invariants(pkg):
     c = k.counters()
     assert c["removals"] == 0 and c["attempts"] == n * L * L
     assert int(s1[0]) - L * L // 2 == 2 * c["deposits"]            # +2 per accepted flip, exactly
-    assert 0.25 < w2[0] < 1.0
+    assert 0.25 < w2[0] < 1.5
     _window_check(pkg, k, L, T, 1.0, 0.0, seed, n, L - 300, L - 300, 600, check_h00=True)   # wraps, holds (0,0)
     _window_check(pkg, k, L, T, 1.0, 0.0, seed, n, 50000, 77777, 512)
     _window_check(pkg, k, L, T, 1.0, 0.0, seed, n, L // 2 - 100, 3, 512)
