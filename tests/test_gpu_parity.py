@@ -511,3 +511,21 @@ def test_run_sampled_config1_times(pkg):
         k.run_sampled([10, 20])            # behind the MCS clock
     with pytest.raises(pkg.KpzError):
         k.run_sampled([70, 70])
+
+
+def test_growth_exponent_loose_sanity(pkg):
+    """Physics sanity, not parity (S:section 4): from the flat start W^2(t) - 1/4 ~ t^(2 beta) with beta_eff(t) =
+    (1/2) log2[(W^2(t) - 1/4) / (W^2(t/2) - 1/4)] (eq. 11 with t/t' = 2 after subtracting 1/4) drifting
+    up towards the paper's beta = 0.2415(15) (P:105) once t > t_mic ~ 50.  One run at L = 2^14, T = 64, p = 1, q = 0;
+    the schedule changes pre-factors, not exponents, so the band is loose."""
+    import math
+    L = 1 << 14
+    k = pkg.KPZ(L, 1.0, 0.0, 64, 42)
+    k.init_flat()
+    times = [64, 128, 256, 512, 1024, 2048]
+    _, _, w2 = k.run_sampled(times)
+    w = w2[:, 0] - 0.25
+    beta = [0.5 * math.log2(w[i] / w[i - 1]) for i in range(1, len(times))]
+    assert all(0.225 < b < 0.255 for b in beta), beta
+    assert all(w[i] > w[i - 1] for i in range(1, len(times)))
+    k.close()
