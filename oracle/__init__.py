@@ -50,6 +50,10 @@ def lib() -> ctypes.CDLL:
         L.kpzo_set_schedule.restype = ci
         L.kpzo_set_sub_sweeps.argtypes = [vp, u32]
         L.kpzo_set_sub_sweeps.restype = ci
+        L.kpzo_set_poisson.argtypes = [vp, ci]
+        L.kpzo_set_poisson.restype = ci
+        L.kpzo_poisson_table.argtypes = [vp, vp, vp]
+        L.kpzo_poisson_table.restype = u32
         L.kpzo_run.argtypes = [vp, u64]
         L.kpzo_run.restype = ci
         L.kpzo_run_checked.argtypes = [vp, u64]
@@ -127,6 +131,19 @@ class Oracle:
         """K sub-sweeps per MCS, each with its own origin shift and colour order (S6)."""
         if lib().kpzo_set_sub_sweeps(self._h, int(K)) != 0:
             raise ValueError("K must divide T*T")
+
+    def set_poisson(self, on=True):
+        """Poissonised number of steps per tile and sub-sweep (S7)."""
+        if lib().kpzo_set_poisson(self._h, int(bool(on))) != 0:
+            raise ValueError("tile*tile/K too large for the Poissonised schedule")
+
+    def poisson_table(self):
+        """(kmin, thresholds) of the S7 count table; thresholds[i] = floor(2^32 P(n <= kmin + i))."""
+        kmin = ctypes.c_uint32()
+        n = lib().kpzo_poisson_table(self._h, ctypes.addressof(kmin), None)
+        thr = np.zeros(n, dtype=np.uint64)
+        lib().kpzo_poisson_table(self._h, ctypes.addressof(kmin), thr.ctypes.data)
+        return kmin.value, thr
 
     def init_flat(self):
         lib().kpzo_init_flat(self._h)

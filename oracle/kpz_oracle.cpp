@@ -84,6 +84,9 @@ struct Oracle {
     uint64_t mcs, attempts, deposits, removals;
     int nthreads;
     uint32_t sub_sweeps;   // K >= 1 sub-sweeps per MCS (S6); K divides T*T
+    bool poisson;          // S7: Poissonised number of steps per tile and sub-sweep
+    uint32_t pk_min;       // smallest count of the table
+    std::vector<uint64_t> pthr;   // pthr[i] = floor(2^32 * P(n <= pk_min + i)), last entry 2^32
     int schedule;      // 0: four tile colours with halo (S4); 1: dead borders, one pass (S5)
 };
 
@@ -139,6 +142,42 @@ void global_draw(const Oracle* o, uint32_t m, uint32_t sub, uint32_t* ox, uint32
     perm[3] = pool[0];
 }
 
+// S7: integer-defined Poisson table for lambda = T*T/K.  Weights q_lambda = 2^52 at the mode, q_k = floor(q_{k-1}
+// * lambda / k) above it and q_k = floor(q_{k+1} * (k+1) / lambda) below it, for |k - lambda| <= W =
+// ceil(12 sqrt(lambda)) + 16 (k >= 0); thresholds floor(2^32 * C_k / S) with C_k the running sum and S the total.
+void build_poisson_table(Oracle* o) {
+    const uint64_t lam = (uint64_t)o->T * o->T / o->sub_sweeps;
+    uint64_t W = 16;
+    while ((W - 16) * (W - 16) < 144 * lam) ++W;              // W - 16 = ceil(12 sqrt(lambda))
+    const uint64_t kmin = lam > W ? lam - W : 0, kmax = lam + W;
+    std::vector<u128> q(kmax - kmin + 1);
+    q[lam - kmin] = (u128)1 << 52;
+    for (uint64_t k = lam + 1; k <= kmax; ++k) q[k - kmin] = q[k - 1 - kmin] * lam / k;
+    for (uint64_t k = lam; k-- > kmin;) q[k - kmin] = q[k + 1 - kmin] * (k + 1) / lam;
+    u128 S = 0;
+    for (u128 v : q) S += v;
+    o->pk_min = (uint32_t)kmin;
+    o->pthr.resize(q.size());
+    u128 C = 0;
+    for (size_t i = 0; i < q.size(); ++i) {
+        C += q[i];
+        o->pthr[i] = (uint64_t)((C << 32) / S);
+    }
+}
+
+// number of steps of tile `tile_id` in sub-sweep `sub` of MCS m: kmin + #{i : pthr[i] <= u}, u = word 0 of the
+// count call R(0x7FFFFFFF - sub, tile_id, m, replica)
+uint32_t poisson_count(const Oracle* o, uint32_t m, uint32_t sub, uint32_t tile_id) {
+    const uint32_t ctr[4] = {0x7FFFFFFFu - sub, tile_id, m, o->replica};
+    const uint32_t key[2] = {(uint32_t)(o->seed & 0xFFFFFFFFu), (uint32_t)(o->seed >> 32)};
+    uint32_t Q[4];
+    philox4x32_10(ctr, key, Q);
+    uint32_t n = o->pk_min;
+    for (size_t i = 0; i + 1 < o->pthr.size(); ++i)
+        if (o->pthr[i] <= (uint64_t)Q[0]) ++n;
+    return n;
+}
+
 // all T*T sequential steps of tile (tx,ty) in MCS m.  DESIGN.md "Schedule" S3.
 void run_tile(Oracle* o, uint32_t m, uint32_t ox, uint32_t oy, uint32_t tx, uint32_t ty,
               uint64_t* n_dep, uint64_t* n_rem, int64_t* dh00, uint32_t s_begin, uint32_t s_end) {
@@ -151,6 +190,14 @@ void run_tile(Oracle* o, uint32_t m, uint32_t ox, uint32_t oy, uint32_t tx, uint
     // step s takes digit s & 1 of word (s >> 1) & 3 of call R(s >> 3, ...); its accept word is word s & 3 of call
     // R((s >> 2) | 0x80000000, ...).
     uint32_t QS[4] = {0, 0, 0, 0}, QA[4] = {0, 0, 0, 0};
+    if (o->poisson) {
+        // S7: sub-sweep j = s_begin / (T*T/K) owns the stream region starting at step j * 2^16 and runs n steps of it
+        const uint32_t sub = s_begin / (steps / o->sub_sweeps);
+        s_begin = sub << 16;
+        s_end = s_begin + poisson_count(o, m, sub, tile_id);
+        #pragma omp atomic
+        o->attempts += (uint64_t)(s_end - s_begin);
+    }
     for (uint32_t s = s_begin; s < s_end; ++s) {
         if ((s & 7u) == 0u || s == s_begin) {
             uint32_t ctr_s[4] = {s >> 3, tile_id, m, o->replica};
@@ -230,7 +277,7 @@ void run_one_mcs(Oracle* o) {
     const uint32_t m = (uint32_t)o->mcs;
     const uint32_t steps = o->T * o->T, K = o->sub_sweeps;
     for (uint32_t j = 0; j < K; ++j) run_sub_sweep(o, m, j, j * (steps / K), (j + 1) * (steps / K));
-    o->attempts += (uint64_t)o->L * o->L;
+    if (!o->poisson) o->attempts += (uint64_t)o->L * o->L;     // S7 counts the steps it really made (run_tile)
     o->mcs += 1;
 }
 
@@ -295,6 +342,7 @@ void* kpzo_create(uint32_t L, double p, double q, uint32_t T, uint64_t seed, uin
     o->thr_p = threshold(p); o->thr_q = threshold(q);
     o->schedule = 0;
     o->sub_sweeps = 1;
+    o->poisson = false; o->pk_min = 0;
     o->full = (ww == 0 && wh == 0);
     if (o->full) { wx0 = wy0 = 0; ww = wh = L; }
     if (ww > L || wh > L) { delete o; return nullptr; }
@@ -345,7 +393,25 @@ int kpzo_set_sub_sweeps(void* h, uint32_t K) {
     Oracle* o = static_cast<Oracle*>(h);
     if (K < 1 || (o->T * o->T) % K != 0) return -1;
     o->sub_sweeps = K;
+    if (o->poisson) build_poisson_table(o);
     return 0;
+}
+
+// S7 on / off.  Needs T*T/K + W < 2^16 (one stream region per sub-sweep).  Returns 0 or -1.
+int kpzo_set_poisson(void* h, int on) {
+    Oracle* o = static_cast<Oracle*>(h);
+    if (on && (uint64_t)o->T * o->T / o->sub_sweeps > 60000) return -1;
+    o->poisson = on != 0;
+    if (o->poisson) build_poisson_table(o);
+    return 0;
+}
+
+// table access for the tests: returns the number of entries, fills kmin and (if thr != NULL) the thresholds
+uint32_t kpzo_poisson_table(void* h, uint32_t* kmin, uint64_t* thr) {
+    Oracle* o = static_cast<Oracle*>(h);
+    if (kmin) *kmin = o->pk_min;
+    if (thr) for (size_t i = 0; i < o->pthr.size(); ++i) thr[i] = o->pthr[i];
+    return (uint32_t)o->pthr.size();
 }
 
 int kpzo_run(void* h, uint64_t n_mcs) {

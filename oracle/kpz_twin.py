@@ -43,11 +43,14 @@ def threshold(prob):
 
 
 class Twin:
-    def __init__(self, L, p, q, T, seed, replica=0, schedule="colours", sub_sweeps=1):
+    def __init__(self, L, p, q, T, seed, replica=0, schedule="colours", sub_sweeps=1, poisson=False):
         assert T >= 1 and L % (2 * T) == 0 and schedule in ("colours", "dead_border")
         assert sub_sweeps >= 1 and (T * T) % sub_sweeps == 0
-        self.schedule, self.K = schedule, sub_sweeps
+        self.schedule, self.K, self.poisson = schedule, sub_sweeps, poisson
+        self.attempts = 0
         self.L, self.T, self.p, self.q, self.seed, self.replica = L, T, p, q, seed, replica
+        if poisson:
+            self._poisson_table()
         self.g = 4 if T % 4 == 0 else 1
         self.key = (seed & MASK, (seed >> 32) & MASK)
         self.thr_p, self.thr_q = threshold(p), threshold(q)
@@ -82,6 +85,28 @@ class Twin:
         if self.trace is not None:
             self.trace.append((x, y, d))
 
+    def _poisson_table(self):
+        """DESIGN.md S7, in Python integers: weights 2^52 at the mode lambda = T^2/K, multiplied / divided down the two
+        sides with floor divisions, over |k - lambda| <= ceil(12 sqrt(lambda)) + 16; thresholds floor(2^32 C_k / S)."""
+        import math
+        lam = self.T * self.T // self.K
+        W = math.isqrt(144 * lam - 1) + 1 + 16 if lam > 0 else 16       # ceil(12 sqrt(lambda)) + 16
+        kmin, kmax = max(0, lam - W), lam + W
+        q = {lam: 1 << 52}
+        for k in range(lam + 1, kmax + 1):
+            q[k] = q[k - 1] * lam // k
+        for k in range(lam - 1, kmin - 1, -1):
+            q[k] = q[k + 1] * (k + 1) // lam
+        S = sum(q.values())
+        self.kmin, self.thr, C = kmin, [], 0
+        for k in range(kmin, kmax + 1):
+            C += q[k]
+            self.thr.append((C << 32) // S)
+
+    def _poisson_count(self, m, sub, tile_id):
+        u = philox4x32_10((0x7FFFFFFF - sub, tile_id, m, self.replica), self.key)[0]
+        return self.kmin + sum(1 for t in self.thr[:-1] if t <= u)
+
     def global_draw(self, m, sub=0):
         G = philox4x32_10((sub, MASK, m, self.replica), self.key)
         n = self.T // self.g
@@ -108,8 +133,12 @@ class Twin:
                 for tiles in passes:
                     for (tx, ty) in tiles:
                         tile_id = ty * NT + tx
-                        s0 = j * T * T // self.K
-                        for s in range(s0, (j + 1) * T * T // self.K):
+                        s0, s1 = j * T * T // self.K, (j + 1) * T * T // self.K
+                        if self.poisson:       # S7: own stream region per sub-sweep, Poissonised length
+                            s0 = j << 16
+                            s1 = s0 + self._poisson_count(m, j, tile_id)
+                        self.attempts += s1 - s0
+                        for s in range(s0, s1):
                             # DESIGN.md S3: a site word is a base-T*T fraction with two digits; step s uses digit
                             # s % 2 of word (s // 2) % 4 of call s // 8; accept word = word s % 4 of call s // 4 + 2^31
                             if s % 8 == 0 or s == s0:

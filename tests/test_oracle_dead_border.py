@@ -88,3 +88,55 @@ def test_sub_sweeps_one_is_the_default_and_bad_values_are_rejected():
     assert a.state_hash() == b.state_hash() != c.state_hash()
     with pytest.raises(ValueError):
         a.set_sub_sweeps(7)
+
+
+def test_poisson_table_is_the_poisson_law():
+    """Schedule S7: the integer-defined count table equals the Poisson(lambda = T*T/K) distribution function to
+    the 2^-32 resolution of its thresholds (scipy's regularised gamma function as the independent reference)."""
+    from scipy.stats import poisson
+    for (T, K) in ((16, 1), (64, 1), (64, 16), (32, 4), (4, 2)):
+        o = Oracle(2 * T, 1.0, 0.0, T, 1)
+        o.set_sub_sweeps(K); o.set_poisson(True)
+        kmin, thr = o.poisson_table()
+        lam = T * T // K
+        cdf = poisson.cdf(kmin + np.arange(len(thr)), lam)
+        assert np.max(np.abs(thr.astype(np.float64) / 2.0 ** 32 - cdf)) < 3e-10
+        assert thr[-1] == 2 ** 32 and np.all(np.diff(thr.astype(np.int64)) >= 0)
+        assert kmin <= lam < kmin + len(thr)
+
+
+@pytest.mark.parametrize("L,T,p,q,K,sched", [(16, 4, 1.0, 0.0, 1, "colours"), (24, 3, 0.6, 0.3, 3, "colours"),
+                                             (32, 8, 0.75, 0.25, 2, "dead_border"), (32, 4, 1.0, 0.0, 4, "colours")])
+def test_poissonised_counts_oracle_equals_twin(L, T, p, q, K, sched):
+    o = Oracle(L, p, q, T, 5)
+    o.set_schedule(sched); o.set_sub_sweeps(K); o.set_poisson(True)
+    o.init_flat(); o.run(3)
+    t = kpz_twin.Twin(L, p, q, T, 5, schedule=sched, sub_sweeps=K, poisson=True)
+    t.init_flat(); t.run(3)
+    sx, sy = o.slopes()
+    tx, ty = t.slopes()
+    assert np.array_equal(sx, np.array(tx)) and np.array_equal(sy, np.array(ty))
+    assert o.measure()[:2] == t.sums() and o.check() == 0
+    assert o.counters()["attempts"] == t.attempts
+    kmin, thr = o.poisson_table()
+    assert kmin == t.kmin and [int(v) for v in thr] == t.thr
+
+
+def test_poissonised_attempt_counts_have_poisson_mean_and_variance():
+    """Per MCS the number of attempts is a sum of NT^2 independent Poisson(T*T) counts: mean L*L, variance L*L."""
+    L, T, n = 64, 8, 400
+    o = Oracle(L, 0.0, 0.0, T, 77)         # p = q = 0: only the counting matters, the surface never changes
+    o.set_poisson(True)
+    o.init_flat()
+    per_mcs = []
+    last = 0
+    for _ in range(n):
+        o.run(1)
+        a = o.counters()["attempts"]
+        per_mcs.append(a - last)
+        last = a
+    per_mcs = np.array(per_mcs, dtype=np.float64)
+    lam = L * L
+    assert abs(per_mcs.mean() - lam) < 4 * np.sqrt(lam / n)
+    assert 0.8 * lam < per_mcs.var(ddof=1) < 1.25 * lam
+    assert o.measure()[2] == 0.25
