@@ -96,6 +96,13 @@ int32_t kpz_set_schedule(kpz_ctx* ctx, int32_t schedule);
  * K times the launches and the tile staging.  K must divide tile*tile/8 (KPZ_EINVAL otherwise). */
 int32_t kpz_set_sub_sweeps(kpz_ctx* ctx, uint32_t K);
 
+/* Second bias-reduction knob (S7): Poissonised number of steps per tile and sub-sweep.  With
+ * on != 0 every tile runs n steps of its stream, n drawn from the (integer-defined) Poisson law of mean
+ * lambda = tile*tile/K with one Philox word per tile and sub-sweep, instead of exactly lambda steps -- the count
+ * statistics of true random-sequential dynamics.  An MCS is then L*L attempts only on average; kpz_counters reports
+ * the attempts really made.  Needs bound buffers (the table lives in the scratch buffer).  Synchronises. */
+int32_t kpz_set_poisson(kpz_ctx* ctx, int32_t on);
+
 /* Height reconstruction (eq. 3) and width (eq. 4).  HOST out-arrays of length n_replicas (any may be NULL).
  * sum_h, sum_h2: exact sums over all sites of h and h^2 with absolute heights anchored by h(0,0) (tracked:
  * 0 at kpz_init_flat, +-2 per accepted flip at site (0,0)).  W2 = (N*sum_h2 - sum_h^2)/N^2, N = L*L, from
@@ -142,7 +149,7 @@ int32_t kpz_set_slopes(kpz_ctx* ctx, uint32_t replica, const int8_t* sx, const i
 int32_t kpz_state_hash(kpz_ctx* ctx, uint32_t replica, uint64_t* out);
 
 /* Per-replica counters since kpz_init_flat (HOST out-pointers, any may be NULL): attempted updates
- * (= mcs * L*L), accepted depositions and removals, tracked height of site (0,0), completed MCS.  Synchronises. */
+ * (= mcs * L*L unless S7 was on), accepted depositions and removals, tracked height of site (0,0), completed MCS.  Synchronises. */
 int32_t kpz_counters(kpz_ctx* ctx, uint32_t replica, uint64_t* attempts, uint64_t* deposits, uint64_t* removals,
                      int64_t* h00, uint64_t* mcs);
 

@@ -21,7 +21,7 @@ exported_symbols = [
     "kpz_workspace_bytes", "kpz_create", "kpz_create_batch", "kpz_bind", "kpz_init_flat", "kpz_run", "kpz_measure",
     "kpz_destroy", "kpz_synchronize", "kpz_last_error", "kpz_get_slopes", "kpz_get_window", "kpz_set_slopes",
     "kpz_state_hash", "kpz_counters", "kpz_export_packed", "kpz_import_packed", "kpz_step_host",
-    "kpz_launch_count", "kpz_philox_selftest", "kpz_profiles", "kpz_power_spectrum", "kpz_set_schedule", "kpz_set_sub_sweeps", "kpz_run_sampled",
+    "kpz_launch_count", "kpz_philox_selftest", "kpz_profiles", "kpz_power_spectrum", "kpz_set_schedule", "kpz_set_sub_sweeps", "kpz_run_sampled", "kpz_set_poisson",
 ]
 
 
@@ -59,6 +59,7 @@ def load_library() -> ctypes.CDLL:
         "kpz_counters": [vp, u32, vp, vp, vp, vp, vp],
         "kpz_run_sampled": [vp, vp, u32, vp, vp, vp],
         "kpz_set_schedule": [vp, i32],
+        "kpz_set_poisson": [vp, i32],
         "kpz_set_sub_sweeps": [vp, u32],
         "kpz_profiles": [vp, u32, vp, vp],
         "kpz_power_spectrum": [vp, u32, vp, vp, vp],
@@ -182,6 +183,10 @@ class KPZ:
     def set_schedule(self, name):
         """kpz_set_schedule: 'colours' (default) or 'dead_border' (the paper's own scheme)."""
         self._check(self._lib.kpz_set_schedule(self._h, {"colours": 0, "dead_border": 1}[name]))
+
+    def set_poisson(self, on=True):
+        """kpz_set_poisson: Poissonised number of steps per tile and sub-sweep (S7)."""
+        self._check(self._lib.kpz_set_poisson(self._h, int(bool(on))))
 
     def set_sub_sweeps(self, K):
         """kpz_set_sub_sweeps: K sub-sweeps per MCS, each with its own origin shift and colour order."""

@@ -32,6 +32,7 @@ struct ScratchLayout {
     size_t fft;       // [2][L] double2
     size_t sdir;      // [2][L/2+1] double
     size_t savg;      // [L/2+1] double
+    size_t ptab;      // [4096] u64     S7 count table
     size_t total;
     uint32_t n_chunks, rows_per_chunk;
 };
@@ -59,6 +60,7 @@ ScratchLayout scratch_layout(uint32_t L, uint32_t R) {
     s.fft = o;    o += align_up((size_t)2 * L * 16, 256);
     s.sdir = o;   o += align_up((size_t)2 * (L / 2 + 1) * 8, 256);
     s.savg = o;   o += align_up((size_t)(L / 2 + 1) * 8, 256);
+    s.ptab = o;   o += 4096 * 8;
     s.total = o;
     return s;
 }
@@ -92,6 +94,9 @@ struct kpz_ctx {
     uint64_t launches;
     int32_t schedule;        // KPZ_SCHEDULE_COLOURS or KPZ_SCHEDULE_DEAD_BORDER
     uint32_t sub_sweeps;     // K sub-sweeps per MCS (S6)
+    bool poisson;            // Poissonised steps per tile and sub-sweep (S7)
+    uint32_t pn, pk_min;     // count table on the device (scratch ptab): entries, smallest count
+    uint64_t attempts_base;  // attempts made by fixed-count MCS (S7 MCS count theirs on the device, stats[3])
     uint32_t* d_lattice;
     unsigned char* d_scratch;
     cudaStream_t stream;
@@ -128,7 +133,7 @@ int grid_for(uint64_t n, int block, int cap = 148 * 16) {
     return (int)g;
 }
 
-template <int T, int NTHR, int MODE, bool DEAD, bool SUB>
+template <int T, int NTHR, int MODE, bool DEAD, int SUB>
 int32_t launch_update_k(kpz_ctx* c, const kpz::UpdateParams& P) {
     const size_t smem = (size_t)kpz::TileGeom<T>::WORDS * NTHR * sizeof(uint32_t);
     auto kern = kpz::kpz_update_kernel<T, NTHR, MODE, DEAD, SUB>;
@@ -148,7 +153,8 @@ int32_t launch_update_k(kpz_ctx* c, const kpz::UpdateParams& P) {
 
 template <int T, int NTHR, int MODE, bool DEAD>
 int32_t launch_update_t(kpz_ctx* c, const kpz::UpdateParams& P) {
-    return c->sub_sweeps > 1 ? launch_update_k<T, NTHR, MODE, DEAD, true>(c, P) : launch_update_k<T, NTHR, MODE, DEAD, false>(c, P);
+    if (c->poisson) return launch_update_k<T, NTHR, MODE, DEAD, 2>(c, P);
+    return c->sub_sweeps > 1 ? launch_update_k<T, NTHR, MODE, DEAD, 1>(c, P) : launch_update_k<T, NTHR, MODE, DEAD, 0>(c, P);
 }
 
 template <int T, int NTHR, bool DEAD>
@@ -186,6 +192,9 @@ int32_t launch_update(kpz_ctx* c, uint32_t m, uint32_t slot, uint32_t sub) {
     const uint32_t calls = c->T * c->T / 8u, per = calls / c->sub_sweeps;
     P.call_begin = sub * per;
     P.call_end = (sub + 1u) * per;
+    P.pthr = reinterpret_cast<const unsigned long long*>(c->d_scratch + c->sl.ptab);
+    P.pn = c->pn;
+    P.pk_min = c->pk_min;
     P.key.k0 = (uint32_t)(c->seed & 0xFFFFFFFFull);
     P.key.k1 = (uint32_t)(c->seed >> 32);
     switch (c->T) {
@@ -270,6 +279,7 @@ int32_t kpz_create_batch(kpz_ctx** out, uint32_t L, double p, double q, uint32_t
     if (!c) return KPZ_ENOMEM;
     c->L = L; c->T = tile; c->R = n_replicas; c->p = p; c->q = q; c->seed = seed;
     c->mcs = 0; c->launches = 0; c->schedule = KPZ_SCHEDULE_COLOURS; c->sub_sweeps = 1;
+    c->poisson = false; c->pn = 0; c->pk_min = 0; c->attempts_base = 0;
     c->d_lattice = nullptr; c->d_scratch = nullptr; c->stream = nullptr; c->bound = false;
     c->sl = scratch_layout(L, n_replicas);
     c->lattice_bytes = (size_t)n_replicas * ((size_t)L * L / 4);
@@ -306,6 +316,7 @@ int32_t kpz_init_flat(kpz_ctx* c) {
     c->launches++;
     KPZ_CUDA(c, cudaMemsetAsync(c->d_scratch + c->sl.stats, 0, (size_t)c->R * 32, c->stream));
     c->mcs = 0;
+    c->attempts_base = 0;
     return KPZ_OK;
 }
 
@@ -323,6 +334,7 @@ int32_t kpz_run(kpz_ctx* c, uint64_t mcs) {
             }
         }
         c->mcs++;
+        if (!c->poisson) c->attempts_base += (uint64_t)c->L * c->L;
     }
     return KPZ_OK;
 }
@@ -334,12 +346,48 @@ int32_t kpz_set_schedule(kpz_ctx* c, int32_t schedule) {
     return KPZ_OK;
 }
 
+static int32_t upload_poisson_table(kpz_ctx* c);
+
 int32_t kpz_set_sub_sweeps(kpz_ctx* c, uint32_t K) {
     if (!c) return KPZ_EINVAL;
     const uint32_t calls = c->T * c->T / 8u;
     if (K < 1 || K > calls || calls % K != 0) return fail(c, KPZ_EINVAL, "sub-sweeps must divide tile*tile/8");
     c->sub_sweeps = K;
+    return (c->poisson && c->bound) ? upload_poisson_table(c) : KPZ_OK;
+}
+
+// S7 table: weights 2^52 at the mode, floor-multiplied down both sides, thresholds in 2^-32
+static int32_t upload_poisson_table(kpz_ctx* c) {
+    const uint64_t lam = (uint64_t)c->T * c->T / c->sub_sweeps;
+    uint64_t W = 0;
+    while (W * W < 144ull * lam) ++W;
+    W += 16;
+    const uint64_t kmin = lam > W ? lam - W : 0, kmax = lam + W, n = kmax - kmin + 1;
+    if (n > 4096) return fail(c, KPZ_EINVAL, "Poisson table too large");
+    std::vector<u128> w(n);
+    w[lam - kmin] = (u128)1 << 52;
+    for (uint64_t k = lam + 1; k <= kmax; ++k) w[k - kmin] = w[k - kmin - 1] * lam / k;
+    for (uint64_t k = lam; k > kmin; --k) w[k - 1 - kmin] = w[k - kmin] * k / lam;
+    u128 total = 0;
+    for (uint64_t i = 0; i < n; ++i) total += w[i];
+    std::vector<unsigned long long> thr(n);
+    u128 run = 0;
+    for (uint64_t i = 0; i < n; ++i) {
+        run += w[i];
+        thr[i] = (unsigned long long)((run << 32) / total);
+    }
+    KPZ_CUDA(c, cudaMemcpyAsync(c->d_scratch + c->sl.ptab, thr.data(), n * 8, cudaMemcpyHostToDevice, c->stream));
+    KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->pn = (uint32_t)n;
+    c->pk_min = (uint32_t)kmin;
     return KPZ_OK;
+}
+
+int32_t kpz_set_poisson(kpz_ctx* c, int32_t on) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    c->poisson = on != 0;
+    return c->poisson ? upload_poisson_table(c) : KPZ_OK;
 }
 
 int32_t kpz_measure(kpz_ctx* c, int64_t* sum_h, int64_t* sum_h2, double* W2) {
@@ -487,7 +535,7 @@ int32_t kpz_counters(kpz_ctx* c, uint32_t replica, uint64_t* attempts, uint64_t*
     unsigned long long st[4];
     KPZ_CUDA(c, cudaMemcpyAsync(st, c->d_scratch + c->sl.stats + (size_t)replica * 32, 32, cudaMemcpyDeviceToHost, c->stream));
     KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
-    if (attempts) *attempts = c->mcs * (uint64_t)c->L * c->L;
+    if (attempts) *attempts = c->attempts_base + st[3];
     if (deposits) *deposits = st[0];
     if (removals) *removals = st[1];
     if (h00) *h00 = (int64_t)st[2];
@@ -512,10 +560,11 @@ int32_t kpz_import_packed(kpz_ctx* c, const void* host_src, size_t bytes, const 
     std::vector<unsigned long long> st((size_t)c->R * 4, 0ull);
     KPZ_CUDA(c, cudaMemcpyAsync(st.data(), c->d_scratch + c->sl.stats, (size_t)c->R * 32, cudaMemcpyDeviceToHost, c->stream));
     KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
-    for (uint32_t r = 0; r < c->R; ++r) st[4 * r + 2] = (unsigned long long)(h00 ? h00[r] : 0);
+    for (uint32_t r = 0; r < c->R; ++r) { st[4 * r + 2] = (unsigned long long)(h00 ? h00[r] : 0); st[4 * r + 3] = 0ull; }
     KPZ_CUDA(c, cudaMemcpyAsync(c->d_scratch + c->sl.stats, st.data(), (size_t)c->R * 32, cudaMemcpyHostToDevice, c->stream));
     KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
     c->mcs = mcs;
+    c->attempts_base = mcs * (uint64_t)c->L * c->L;
     return KPZ_OK;
 }
 

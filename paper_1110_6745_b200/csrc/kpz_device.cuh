@@ -56,7 +56,7 @@ __device__ __forceinline__ uint32_t mulhi32(uint32_t a, uint32_t n) { return __u
 // ------------------------------------------------------------------------------------------------------------
 struct UpdateParams {
     uint32_t* lattice;             // device: packed lattice, all replicas
-    unsigned long long* stats;     // device: [R][4] = deposits, removals, h00 (two's complement), reserved
+    unsigned long long* stats;     // device: [R][4] = deposits, removals, h00 (two's complement), attempts made under S7
     uint64_t plane_words;          // L*L/32
     uint64_t total_items;          // R * HN*HN  (tiles of one colour over all replicas)
     uint64_t thr_p, thr_q;         // accept iff (uint64)word < thr
@@ -69,6 +69,8 @@ struct UpdateParams {
     uint32_t slot;                 // 0..3: which entry of the colour order this launch executes
     uint32_t sub;                  // sub-sweep index j (S6): counter word c0 of the global draw
     uint32_t call_begin, call_end; // site calls [call_begin, call_end) of every tile: steps 8*call_begin .. 8*call_end
+    const unsigned long long* pthr; // S7: device table, pthr[i] = floor(2^32 P(n <= pk_min + i)), pn entries
+    uint32_t pn, pk_min;
     PhiloxKey key;
 };
 
@@ -428,7 +430,7 @@ __device__ __forceinline__ uint32_t lop3_and_not_not(uint32_t m, uint32_t x, uin
 template <int T, int NTHR, int MODE, bool TRACK, bool DEAD>
 __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site_word, uint32_t accept_word,
                                         const UpdateParams& P, uint32_t& n_dep, uint32_t& n_rem, int32_t& dh00,
-                                        uint32_t origin_idx) {
+                                        uint32_t origin_idx, bool live = true) {
     using G = TileGeom<T>;
     const uint32_t idx = site_word >> (32 - 2 * G::LOG2T);      // mulhi32(site_word, T*T) = ly*T + lx
     const uint32_t ly = idx >> G::LOG2T;
@@ -460,6 +462,7 @@ __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site
         const bool edge = (((idx + 1u) & (uint32_t)(T - 1)) == 0u) || (idx >= (uint32_t)(T * (T - 1)));
         bit = edge ? 0u : bit;
     }
+    bit = live ? bit : 0u;      // S7: steps beyond the tile's Poissonised count (constant true elsewhere)
     // local minimum <=> no neighbour differs from v
     const uint32_t md0 = lop3_and_not_not(bit, lop3_any_differs(v, wl, wr), lop3_any_differs(v, wd, wu));
     if (MODE == 0) {
@@ -495,14 +498,17 @@ __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site
 // evaluated only in MODE 1.  Calls are generated one batch ahead of the attempts that consume them (the generator
 // is counter-based, so the next batch does not depend on the lattice): the multiplier pipe works on batch b+1
 // while the shared-memory round trips of batch b are in flight.
-template <int T, int NTHR, int MODE, bool TRACK, bool DEAD, bool WHOLE>
+template <int T, int NTHR, int MODE, bool TRACK, bool DEAD, int SUBM>
 __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const UpdateParams& P, uint32_t tile_id,
                                                uint32_t replica, uint32_t& n_dep, uint32_t& n_rem, int32_t& dh00,
-                                               uint32_t origin_idx) {
+                                               uint32_t origin_idx, uint32_t n_steps) {
+    constexpr bool WHOLE = (SUBM == 0);
     constexpr uint32_t ACCEPT = 0x80000000u;
     constexpr uint32_t TT = (uint32_t)(T * T);
     // WHOLE: all T*T/8 site calls of the tile (compile-time trip count); otherwise one sub-sweep's slice (S6)
-    const uint32_t c_begin = WHOLE ? 0u : P.call_begin, c_end = WHOLE ? (uint32_t)(T * T) / 8u : P.call_end;
+    // SUBM 2 (S7): the sub-sweep's own stream region (steps from sub * 2^16), n_steps of them for this tile
+    const uint32_t c_begin = WHOLE ? 0u : (SUBM == 2 ? (P.sub << 13) : P.call_begin);
+    const uint32_t c_end = WHOLE ? (uint32_t)(T * T) / 8u : (SUBM == 2 ? c_begin + ((n_steps + 7u) >> 3) : P.call_end);
     uint4 cur, nxt, cur_a[2], nxt_a[2];
     cur = philox4x32_10(c_begin, tile_id, P.m, replica, P.key);
     if (MODE) {
@@ -520,16 +526,17 @@ __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const 
             nxt_a[0] = philox4x32_10((2u * c + 2u) | ACCEPT, tile_id, P.m, replica, P.key);
             nxt_a[1] = philox4x32_10((2u * c + 3u) | ACCEPT, tile_id, P.m, replica, P.key);
         }
+        const uint32_t rem = n_steps - 8u * (c - c_begin);      // S7: live steps left in this call and after
         const uint4 a0 = MODE ? cur_a[0] : make_uint4(0u, 0u, 0u, 0u);
         const uint4 a1 = MODE ? cur_a[1] : make_uint4(0u, 0u, 0u, 0u);
-        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.x, a0.x, P, n_dep, n_rem, dh00, origin_idx);
-        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.x * TT, a0.y, P, n_dep, n_rem, dh00, origin_idx);
-        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.y, a0.z, P, n_dep, n_rem, dh00, origin_idx);
-        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.y * TT, a0.w, P, n_dep, n_rem, dh00, origin_idx);
-        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.z, a1.x, P, n_dep, n_rem, dh00, origin_idx);
-        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.z * TT, a1.y, P, n_dep, n_rem, dh00, origin_idx);
-        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.w, a1.z, P, n_dep, n_rem, dh00, origin_idx);
-        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.w * TT, a1.w, P, n_dep, n_rem, dh00, origin_idx);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.x, a0.x, P, n_dep, n_rem, dh00, origin_idx, SUBM != 2 || rem > 0u);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.x * TT, a0.y, P, n_dep, n_rem, dh00, origin_idx, SUBM != 2 || rem > 1u);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.y, a0.z, P, n_dep, n_rem, dh00, origin_idx, SUBM != 2 || rem > 2u);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.y * TT, a0.w, P, n_dep, n_rem, dh00, origin_idx, SUBM != 2 || rem > 3u);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.z, a1.x, P, n_dep, n_rem, dh00, origin_idx, SUBM != 2 || rem > 4u);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.z * TT, a1.y, P, n_dep, n_rem, dh00, origin_idx, SUBM != 2 || rem > 5u);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.w, a1.z, P, n_dep, n_rem, dh00, origin_idx, SUBM != 2 || rem > 6u);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.w * TT, a1.w, P, n_dep, n_rem, dh00, origin_idx, SUBM != 2 || rem > 7u);
         cur = nxt;
         if (MODE) {
             cur_a[0] = nxt_a[0];
@@ -540,8 +547,9 @@ __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const 
 
 // DEAD = false: one colour of schedule S4 per launch (P.slot);  DEAD = true: every tile of the dead-border schedule
 // S5 in one launch (P.HN = NT).
-// SUB = true: one sub-sweep (S6), site calls [P.call_begin, P.call_end) of every tile instead of all of them.
-template <int T, int NTHR, int MODE, bool DEAD, bool SUB>
+// SUB = 1: one sub-sweep (S6), site calls [P.call_begin, P.call_end) of every tile instead of all of them.
+// SUB = 2: Poissonised number of steps per tile (S7), drawn here from the count call and the table P.pthr.
+template <int T, int NTHR, int MODE, bool DEAD, int SUB>
 // T = 64: 8 CTAs fit the shared memory; asking for 10 caps the registers at 204, which measured best on B200
 // (168, ptxas' own choice: -1.5 %; 255: -1.5 %)
 __global__ void __launch_bounds__(NTHR, (T == 64) ? 10 : 1) kpz_update_kernel(const UpdateParams P) {
@@ -577,7 +585,7 @@ __global__ void __launch_bounds__(NTHR, (T == 64) ? 10 : 1) kpz_update_kernel(co
     const uint32_t x0 = (X0 >= L) ? X0 - L : X0;   // first own column = bit offset inside a row
     const uint32_t y0 = (Y0 >= L) ? Y0 - L : Y0;   // first own row
 
-    uint32_t n_dep = 0, n_rem = 0;
+    uint32_t n_dep = 0, n_rem = 0, n_att = 0;
     int32_t dh00 = 0;
     uint32_t origin_idx = 0xFFFFFFFFu;
     if (active) {
@@ -592,10 +600,22 @@ __global__ void __launch_bounds__(NTHR, (T == 64) ? 10 : 1) kpz_update_kernel(co
     const bool any_origin = __any_sync(0xFFFFFFFFu, origin_idx != 0xFFFFFFFFu);
     if (active) {
         // ---- a3 + a4: T*T sequential attempts ----
+        uint32_t n_steps = 0u;
+        if (SUB == 2) {
+            // n = pk_min + #{i < pn - 1 : pthr[i] <= u}: upper bound in the monotone table
+            const uint32_t u = philox4x32_10(0x7FFFFFFFu - P.sub, tile_id, P.m, replica, P.key).x;
+            uint32_t lo = 0u, hi = P.pn - 1u;
+            while (lo < hi) {
+                const uint32_t mid = (lo + hi) >> 1;
+                if (P.pthr[mid] <= (unsigned long long)u) lo = mid + 1u; else hi = mid;
+            }
+            n_steps = P.pk_min + lo;
+            n_att = n_steps;
+        }
         if (any_origin)
-            run_tile_steps<T, NTHR, MODE, true, DEAD, !SUB>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx);
+            run_tile_steps<T, NTHR, MODE, true, DEAD, SUB>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx, n_steps);
         else
-            run_tile_steps<T, NTHR, MODE, false, DEAD, !SUB>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx);
+            run_tile_steps<T, NTHR, MODE, false, DEAD, SUB>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx, n_steps);
         // ---- a5: write back ----
         if constexpr (G::WIDE) stage_out_wide<T, NTHR, StageBatch<T>::N, DEAD>(planeX, planeY, L, W, x0, y0, sm);
         else stage_out_narrow<T, NTHR, DEAD>(planeX, planeY, L, W, x0, y0, sm);
@@ -604,25 +624,28 @@ __global__ void __launch_bounds__(NTHR, (T == 64) ? 10 : 1) kpz_update_kernel(co
     const uint32_t rep0 = __shfl_sync(0xFFFFFFFFu, replica, 0);
     const bool uniform = __all_sync(0xFFFFFFFFu, replica == rep0 && active);
     if (uniform) {
-        uint32_t d = n_dep, r = n_rem;
+        uint32_t d = n_dep, r = n_rem, a = n_att;
         int32_t h = dh00;
 #pragma unroll
         for (int sft = 16; sft > 0; sft >>= 1) {
             d += __shfl_xor_sync(0xFFFFFFFFu, d, sft);
             r += __shfl_xor_sync(0xFFFFFFFFu, r, sft);
             h += __shfl_xor_sync(0xFFFFFFFFu, h, sft);
+            if (SUB == 2) a += __shfl_xor_sync(0xFFFFFFFFu, a, sft);
         }
         if ((threadIdx.x & 31u) == 0u) {
             unsigned long long* st = P.stats + (size_t)rep0 * 4u;
             if (d) atomicAdd(st + 0, (unsigned long long)d);
             if (r) atomicAdd(st + 1, (unsigned long long)r);
             if (h) atomicAdd(st + 2, (unsigned long long)(long long)h);
+            if (SUB == 2 && a) atomicAdd(st + 3, (unsigned long long)a);
         }
     } else if (active) {
         unsigned long long* st = P.stats + (size_t)replica * 4u;
         if (n_dep) atomicAdd(st + 0, (unsigned long long)n_dep);
         if (n_rem) atomicAdd(st + 1, (unsigned long long)n_rem);
         if (dh00) atomicAdd(st + 2, (unsigned long long)(long long)dh00);
+        if (SUB == 2 && n_att) atomicAdd(st + 3, (unsigned long long)n_att);
     }
 }
 

@@ -529,3 +529,33 @@ def test_growth_exponent_loose_sanity(pkg):
     assert all(0.225 < b < 0.255 for b in beta), beta
     assert all(w[i] > w[i - 1] for i in range(1, len(times)))
     k.close()
+
+
+@pytest.mark.parametrize("L,T,p,q,K,sched,seed", [
+    (64, 8, 1.0, 0.0, 1, "colours", 51),
+    (96, 16, 0.75, 0.25, 4, "colours", 52),
+    (128, 32, 1.0, 0.0, 2, "dead_border", 53),
+    (512, 64, 1.0, 0.0, 1, "colours", 54),
+    (512, 64, 0.6, 0.2, 16, "colours", 55),
+])
+def test_poissonised_counts_parity(pkg, L, T, p, q, K, sched, seed):
+    """Schedule S7: Poissonised number of steps per tile and sub-sweep; bit-exact state, sums and counters
+    (including the number of attempts really made)."""
+    k = pkg.KPZ(L, p, q, T, seed)
+    k.set_schedule(sched); k.set_sub_sweeps(K); k.set_poisson(True)
+    k.init_flat()
+    o = Oracle(L, p, q, T, seed, threads=NTHREADS)
+    o.set_schedule(sched); o.set_sub_sweeps(K); o.set_poisson(True)
+    o.init_flat()
+    for t in range(3):
+        k.run(1); o.run(1)
+        _compare_full(k, o)
+        _compare_scalars(k, [o])
+    assert k.counters()["attempts"] != 3 * L * L or L <= 64
+    # back to fixed counts: the attempts counter continues with exactly L*L per MCS
+    k.set_poisson(False); o.set_poisson(False)
+    a0 = k.counters()["attempts"]
+    k.run(1); o.run(1)
+    _compare_full(k, o)
+    _compare_scalars(k, [o])
+    assert k.counters()["attempts"] == a0 + L * L
