@@ -146,6 +146,20 @@ __device__ __forceinline__ uint32_t prefix_xor32(uint32_t t) {
     return t;
 }
 
+// Parity-free encoding of the T >= 32 tile: shared memory holds u = h1 ^ E with
+//   E(x,y) = ((x + (y&1)) >> 1 & 1) ^ (y >> 1 & 1)      (period 4 in x and y; words start at multiples of 32),
+// chosen so that the test of eq. 2 needs no parity word:
+//   local minimum  <=>  u(x+1,y) == u, u(x-1,y) != u, u(x,y+1) == u, u(x,y-1) != u;   local maximum: all four reversed.
+// enc_word(ly): E over the 32 columns of an own word of row ly;  enc_halo(ly): E of the two used bits of the halo
+// word H_ly (bit 0 = column T of row ly, bit 31 = column -1 of row ly+1).  ly = -1 is 0xFFFFFFFF (== 3 mod 4).
+__device__ __forceinline__ uint32_t enc_word(uint32_t ly) {
+    return ((ly & 1u) ? 0x66666666u : 0xCCCCCCCCu) ^ (0u - ((ly >> 1) & 1u));
+}
+__device__ __forceinline__ uint32_t enc_halo(uint32_t ly) {
+    const uint32_t y1 = ly + 1u;
+    return ((ly >> 1) & 1u) | ((((y1 & 1u) ^ 1u) ^ ((y1 >> 1) & 1u)) << 31);
+}
+
 // ---- a2: stage tile + halo, slopes (HBM) -> height bits (shared memory), T >= 32 -----------------------------
 template <int T, int NTHR, int NB = StageBatch<T>::N>
 __device__ __forceinline__ void stage_in_wide(const uint32_t* __restrict__ planeX, const uint32_t* __restrict__ planeY,
@@ -202,7 +216,7 @@ __device__ __forceinline__ void stage_in_wide(const uint32_t* __restrict__ plane
                 for (int k = 0; k < WPL; ++k) {
                     const uint32_t yv = __funnelshift_r(ry[b][k], ry[b][k + 1], s);
                     cur[k] = prev[k];
-                    sm[(G::PAD + k) * NTHR] = prev[k] ^ yv ^ yc;
+                    sm[(G::PAD + k) * NTHR] = prev[k] ^ yv ^ yc ^ enc_word(0xFFFFFFFFu);
                 }
             } else {
 #pragma unroll
@@ -212,16 +226,16 @@ __device__ __forceinline__ void stage_in_wide(const uint32_t* __restrict__ plane
                 }
             }
 #pragma unroll
-            for (int k = 0; k < WPL; ++k) sm[(G::PAD + r * G::WPR + k) * NTHR] = cur[k];
+            for (int k = 0; k < WPL; ++k) sm[(G::PAD + r * G::WPR + k) * NTHR] = cur[k] ^ enc_word(ly);
             if (ly < (uint32_t)T) {
                 // halos of this row from sigma_x(x0, y) and sigma_x(x0+T, y):  h1(A) = h1(B) ^ sigma ^ (ly & 1)
                 const uint32_t bL = (rx[b][0] >> s) & 1u, bR = (rx[b][1] >> s) & 1u;
                 const uint32_t hL = (cur[0] ^ bL ^ ly) & 1u;
                 const uint32_t hR = ((cur[WPL - 1] >> 31) ^ bR ^ ly) & 1u;
-                sm[(G::PAD + (r - 1u) * G::WPR + WPL) * NTHR] = pendingH | (hL << 31);
+                sm[(G::PAD + (r - 1u) * G::WPR + WPL) * NTHR] = (pendingH | (hL << 31)) ^ enc_halo(ly - 1u);
                 pendingH = hR;
             } else {
-                sm[(G::PAD + (r - 1u) * G::WPR + WPL) * NTHR] = pendingH;
+                sm[(G::PAD + (r - 1u) * G::WPR + WPL) * NTHR] = pendingH ^ enc_halo(ly - 1u);
             }
 #pragma unroll
             for (int k = 0; k < WPL; ++k) prev[k] = cur[k];
@@ -269,8 +283,8 @@ __device__ __forceinline__ void stage_out_wide(uint32_t* __restrict__ planeX, ui
             uint32_t cur[WPL], below[WPL];
 #pragma unroll
             for (int k = 0; k < WPL; ++k) {
-                cur[k] = sm[(G::PAD + r * G::WPR + k) * NTHR];
-                below[k] = sm[(G::PAD + (r - 1u) * G::WPR + k) * NTHR];
+                cur[k] = sm[(G::PAD + r * G::WPR + k) * NTHR] ^ enc_word(ly);
+                below[k] = sm[(G::PAD + (r - 1u) * G::WPR + k) * NTHR] ^ enc_word(ly - 1u);
             }
             // sigma_y(.,ly): T bits at bit offset x0
             {
@@ -298,8 +312,8 @@ __device__ __forceinline__ void stage_out_wide(uint32_t* __restrict__ planeX, ui
             }
             // sigma_x(.,ly): T+1 bits (lx = 0..T) at bit offset x0; rows 0..T-1 only
             if (ly < (uint32_t)T) {
-                const uint32_t hprev = sm[(G::PAD + (r - 1u) * G::WPR + WPL) * NTHR];   // bit 31 = h1(-1, ly)
-                const uint32_t hcur = sm[(G::PAD + r * G::WPR + WPL) * NTHR];           // bit 0  = h1(T, ly)
+                const uint32_t hprev = sm[(G::PAD + (r - 1u) * G::WPR + WPL) * NTHR] ^ enc_halo(ly - 1u);   // bit 31 = h1(-1, ly)
+                const uint32_t hcur = sm[(G::PAD + r * G::WPR + WPL) * NTHR] ^ enc_halo(ly);               // bit 0  = h1(T, ly)
                 const uint32_t xc = ycode(ly);      // bit j = (j + ly) & 1 = h0(lx, ly)
                 uint32_t v[WPL];
 #pragma unroll
@@ -427,6 +441,13 @@ __device__ __forceinline__ uint32_t lop3_and_not_not(uint32_t m, uint32_t x, uin
     return r;
 }
 
+template <int LUT>
+__device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t r;   // bitwise function of (a, b, c) with truth table LUT (a = 0xF0, b = 0xCC, c = 0xAA)
+    asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(r) : "r"(a), "r"(b), "r"(c), "n"(LUT));
+    return r;
+}
+
 template <int T, int NTHR, int MODE, bool TRACK, bool DEAD>
 __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site_word, uint32_t accept_word,
                                         const UpdateParams& P, uint32_t& n_dep, uint32_t& n_rem, int32_t& dh00,
@@ -435,7 +456,7 @@ __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site
     const uint32_t idx = site_word >> (32 - 2 * G::LOG2T);      // mulhi32(site_word, T*T) = ly*T + lx
     const uint32_t ly = idx >> G::LOG2T;
     uint32_t* a;
-    uint32_t wo, wl, wr, sh, par;
+    uint32_t wo, wl, wr, sh;
     if constexpr (G::WIDE) {
         // word (row ly+1, k = lx>>5) = PAD + (ly+1)*WPR + k, and idx>>5 = ly*WPL + k
         a = sm + ((idx >> 5) + ly + (uint32_t)(G::PAD + G::WPR)) * NTHR;
@@ -444,18 +465,14 @@ __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site
         wl = __funnelshift_l(wp, wo, 1);      // left neighbours aligned with their site
         wr = __funnelshift_r(wo, wn, 1);      // right neighbours
         sh = idx;                             // low 5 bits = lx & 31
-        par = ly;
     } else {
         a = sm + (ly + 1u) * NTHR;
         wo = a[0];
         wl = wo << 1;
         wr = wo >> 1;
         sh = (idx & (uint32_t)(T - 1)) + 1u;
-        par = ly + 1u;
     }
     const uint32_t wd = *(a - G::WPR * NTHR), wu = a[G::WPR * NTHR];
-    // v: bit = own_h1 ^ pi at every position of the word (rotation of 0xAAAAAAAA by the row parity)
-    const uint32_t v = wo ^ __funnelshift_r(0xAAAAAAAAu, 0xAAAAAAAAu, par);
     uint32_t bit = __funnelshift_l(0u, 1u, sh);                 // 1 << (sh & 31)
     if (DEAD) {
         // dead-border schedule S5: an attempt on the +x or +y edge of the tile does nothing
@@ -463,16 +480,33 @@ __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site
         bit = edge ? 0u : bit;
     }
     bit = live ? bit : 0u;      // S7: steps beyond the tile's Poissonised count (constant true elsewhere)
-    // local minimum <=> no neighbour differs from v
-    const uint32_t md0 = lop3_and_not_not(bit, lop3_any_differs(v, wl, wr), lop3_any_differs(v, wd, wu));
+    uint32_t md0, mr0 = 0u;     // site bit if the site is a local minimum / maximum, else 0
+    if constexpr (G::WIDE) {
+        // parity-free encoding (enc_word): minimum <=> right, up equal the site's bit and left, down differ
+        md0 = lop3_and_not_not(bit, lop3<0xDB>(wo, wl, wr), lop3<0xBD>(wo, wu, wd));        // (o^~l)|(o^r), (o^u)|(o^~d)
+        if (MODE != 0) mr0 = lop3_and_not_not(bit, lop3<0xBD>(wo, wl, wr), lop3<0xDB>(wo, wu, wd));
+    } else {
+        // v: bit = own_h1 ^ pi at every position of the word (rotation of 0xAAAAAAAA by the row parity)
+        const uint32_t v = wo ^ __funnelshift_r(0xAAAAAAAAu, 0xAAAAAAAAu, ly + 1u);
+        // local minimum <=> no neighbour differs from v;  local maximum <=> all four differ
+        md0 = lop3_and_not_not(bit, lop3_any_differs(v, wl, wr), lop3_any_differs(v, wd, wu));
+        if (MODE != 0) mr0 = lop3_and3(bit, lop3_all_differ(v, wl, wr), lop3_all_differ(v, wd, wu));
+    }
     if (MODE == 0) {
         atomicXor(a, md0);
+#ifdef KPZ_X_FCNT
+        {
+            float cf = __uint_as_float(n_dep);
+            asm("{ .reg .pred p; setp.ne.u32 p, %1, 0; @p add.f32 %0, %0, 0f3F800000; }" : "+f"(cf) : "r"(md0));
+            n_dep = __float_as_uint(cf);
+        }
+#else
         n_dep += (md0 != 0u) ? 1u : 0u;
+#endif
         if (TRACK) dh00 += (md0 != 0u && idx == origin_idx) ? 2 : 0;
     } else if (MODE == 1) {
         // both probabilities > 0: 32-bit inclusive thresholds.  A site is a minimum or a maximum, never both: the
         // threshold is chosen by the site type, one compare decides.
-        const uint32_t mr0 = lop3_and3(bit, lop3_all_differ(v, wl, wr), lop3_all_differ(v, wd, wu));
         const bool is_min = md0 != 0u;
         const bool ok = accept_word <= (is_min ? P.tp_incl : P.tq_incl);
         const uint32_t m = ok ? (md0 | mr0) : 0u;
@@ -482,7 +516,6 @@ __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site
         if (TRACK) dh00 += (idx == origin_idx && m != 0u) ? (is_min ? 2 : -2) : 0;
     } else {
         // general thresholds (a probability of exactly 0 with the other one in (0,1])
-        const uint32_t mr0 = lop3_and3(bit, lop3_all_differ(v, wl, wr), lop3_all_differ(v, wd, wu));
         const uint32_t md = ((uint64_t)accept_word < P.thr_p) ? md0 : 0u;
         const uint32_t mr = ((uint64_t)accept_word < P.thr_q) ? mr0 : 0u;
         atomicXor(a, md | mr);
@@ -552,7 +585,7 @@ __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const 
 template <int T, int NTHR, int MODE, bool DEAD, int SUB>
 // T = 64: 8 CTAs fit the shared memory; asking for 10 caps the registers at 204, which measured best on B200
 // (168, ptxas' own choice: -1.5 %; 255: -1.5 %)
-__global__ void __launch_bounds__(NTHR, (T == 64) ? 10 : 1) kpz_update_kernel(const UpdateParams P) {
+__global__ void __launch_bounds__(NTHR, (T == 64) ? (NTHR == 32 ? 10 : (NTHR == 96 ? 3 : 1)) : 1) kpz_update_kernel(const UpdateParams P) {
     using G = TileGeom<T>;
     extern __shared__ uint32_t smem[];
     uint32_t* sm = smem + threadIdx.x;
@@ -621,6 +654,9 @@ __global__ void __launch_bounds__(NTHR, (T == 64) ? 10 : 1) kpz_update_kernel(co
         else stage_out_narrow<T, NTHR, DEAD>(planeX, planeY, L, W, x0, y0, sm);
     }
     // ---- a6: bookkeeping ----
+#ifdef KPZ_X_FCNT
+    if (MODE == 0) n_dep = (uint32_t)__uint_as_float(n_dep);
+#endif
     const uint32_t rep0 = __shfl_sync(0xFFFFFFFFu, replica, 0);
     const bool uniform = __all_sync(0xFFFFFFFFu, replica == rep0 && active);
     if (uniform) {
