@@ -31,11 +31,12 @@ MCS_PER_STEP = 10
 WORKLOAD = dict(L=1 << 17, tile=64, p=1.0, q=0.0, seed=42)
 
 # Algorithmic work per attempted update on the binding pipe, for p = 1, q = 0:
-# ALU-pipe operations (LOP3 / SHF / LEA / IADD; 16 lanes per clock per scheduler):
+# ALU-pipe operations (LOP3 / SHF / LEA; 16 lanes per clock per scheduler):
 #   1/8 Philox4x32-10 call = 2.5 three-input XORs  (its 2.5 32x32->64 multiplies run on the FMA pipe)
-#   + 12 for the attempt: row index, word address, parity word, own^parity, 2 neighbour alignments,
-#     site bit (2), 2 neighbour tests, mask, count.
-ALG_ALU_OPS_PER_UPDATE = 14.5
+#   + 9 for the attempt: row index, word index, site index, site bit, 2 neighbour alignments, 2 neighbour tests, mask
+#   (the parity-free tile encoding needs no parity word; the address multiply-add and the deposit count run on
+#   the FMA pipe).  Hand count of the minimal sequence for this data layout; the SASS executes 11.4.
+ALG_ALU_OPS_PER_UPDATE = 11.5
 ALG_MUL_OPS_PER_UPDATE = 2.5
 ALG_BYTES_PER_UPDATE = 0.5          # each site (2 bits) read once and written once per MCS
 # dram__bytes_read.sum + dram__bytes_write.sum of one update launch at L = 2^17 (profiles/, ncu --set full)
@@ -199,7 +200,7 @@ def run_ours(args):
     general = not (w["p"] >= 1.0 and w["q"] <= 0.0)
     roofline = {"bound": "alu", "achieved": achieved_tops, "peak": alu_peak_tops, "unit": "Tops/s (ALU-pipe lane-ops)",
                 "frac": achieved_tops / alu_peak_tops, "traffic": TRAFFIC_BYTES_PER_LAUNCH if L == (1 << 17) else None,
-                "kernel": "kpz_update_kernel<%d,%d,%d>" % (T, 32 if T == 64 else 64, 1 if general else 0),
+                "kernel": "kpz_update_kernel<%d,%d,%d>" % (T, 96 if T == 64 else 64, 1 if general else 0),
                 "alg_alu_ops_per_update": ALG_ALU_OPS_PER_UPDATE, "alg_mul_ops_per_update": ALG_MUL_OPS_PER_UPDATE,
                 "launch_ms": upd_launch_ms, "updates_per_launch": upd_per_launch,
                 "peak_source": "148 SM x 4 schedulers x 16 ALU lanes/clk x clocks.max.sm from MEASURED_PEAKS.json "

@@ -198,7 +198,7 @@ int32_t launch_update(kpz_ctx* c, uint32_t m, uint32_t slot, uint32_t sub) {
     P.key.k0 = (uint32_t)(c->seed & 0xFFFFFFFFull);
     P.key.k1 = (uint32_t)(c->seed >> 32);
     switch (c->T) {
-        case 64: return launch_update_mode<64, 32>(c, P);
+        case 64: return launch_update_mode<64, 96>(c, P);
         case 32: return launch_update_mode<32, 64>(c, P);
         case 16: return launch_update_mode<16, 128>(c, P);
         case 8: return launch_update_mode<8, 128>(c, P);

@@ -27,6 +27,6 @@ def test_roofline_constants_match_design():
     import bench
     assert bench.WORKLOAD == dict(L=1 << 17, tile=64, p=1.0, q=0.0, seed=42)      # BASELINE config 3
     assert bench.MCS_PER_STEP * 10 == 100                                         # default K = 10 steps = 100 MCS
-    assert bench.ALG_BYTES_PER_UPDATE == 0.5 and bench.ALG_ALU_OPS_PER_UPDATE == 14.5
+    assert bench.ALG_BYTES_PER_UPDATE == 0.5 and bench.ALG_ALU_OPS_PER_UPDATE == 11.5
     design = (ROOT / "DESIGN.md").read_text()
-    assert "**14.5**" in design and "18.6 T lane-ops/s" in design
+    assert "**11.5**" in design and "18.6 T lane-ops/s" in design
