@@ -451,7 +451,7 @@ __device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c) {
 template <int T, int NTHR, int MODE, bool TRACK, bool DEAD>
 __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site_word, uint32_t accept_word,
                                         const UpdateParams& P, uint32_t& n_dep, float& dep_f, uint32_t& n_rem,
-                                        int32_t& dh00, uint32_t origin_idx, bool live = true) {
+                                        float& rem_f, int32_t& dh00, uint32_t origin_idx, bool live = true) {
     using G = TileGeom<T>;
     const uint32_t idx = site_word >> (32 - 2 * G::LOG2T);      // mulhi32(site_word, T*T) = ly*T + lx
     const uint32_t ly = idx >> G::LOG2T;
@@ -480,38 +480,49 @@ __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site
         bit = edge ? 0u : bit;
     }
     bit = live ? bit : 0u;      // S7: steps beyond the tile's Poissonised count (constant true elsewhere)
-    uint32_t md0, mr0 = 0u;     // site bit if the site is a local minimum / maximum, else 0
+    // min_mask(b) / max_mask(b): b where the site is a local minimum / maximum, else 0
+    uint32_t t1, t2, u1 = 0u, u2 = 0u;
     if constexpr (G::WIDE) {
         // parity-free encoding (enc_word): minimum <=> right, up equal the site's bit and left, down differ
-        md0 = lop3_and_not_not(bit, lop3<0xDB>(wo, wl, wr), lop3<0xBD>(wo, wu, wd));        // (o^~l)|(o^r), (o^u)|(o^~d)
-        if (MODE != 0) mr0 = lop3_and_not_not(bit, lop3<0xBD>(wo, wl, wr), lop3<0xDB>(wo, wu, wd));
+        t1 = lop3<0xDB>(wo, wl, wr);      // (o^~l)|(o^r): not a minimum along x
+        t2 = lop3<0xBD>(wo, wu, wd);      // (o^u)|(o^~d): not a minimum along y
+        if (MODE != 0) {
+            u1 = lop3<0xBD>(wo, wl, wr);  // not a maximum along x
+            u2 = lop3<0xDB>(wo, wu, wd);  // not a maximum along y
+        }
     } else {
         // v: bit = own_h1 ^ pi at every position of the word (rotation of 0xAAAAAAAA by the row parity)
         const uint32_t v = wo ^ __funnelshift_r(0xAAAAAAAAu, 0xAAAAAAAAu, ly + 1u);
-        // local minimum <=> no neighbour differs from v;  local maximum <=> all four differ
-        md0 = lop3_and_not_not(bit, lop3_any_differs(v, wl, wr), lop3_any_differs(v, wd, wu));
-        if (MODE != 0) mr0 = lop3_and3(bit, lop3_all_differ(v, wl, wr), lop3_all_differ(v, wd, wu));
+        t1 = lop3_any_differs(v, wl, wr);         // minimum <=> no neighbour differs from v
+        t2 = lop3_any_differs(v, wd, wu);
+        if (MODE != 0) {
+            u1 = ~lop3_all_differ(v, wl, wr);     // maximum <=> all four differ
+            u2 = ~lop3_all_differ(v, wd, wu);
+        }
     }
     if (MODE == 0) {
+        const uint32_t md0 = lop3_and_not_not(bit, t1, t2);
         atomicXor(a, md0);
         // deposits of this tile counted in fp32 (exact: at most T*T < 2^24 per tile and launch): the predicated
         // FADD runs on the FMA pipe, the integer pipe is the busy one
         asm("{ .reg .pred p; setp.ne.u32 p, %1, 0; @p add.f32 %0, %0, 0f3F800000; }" : "+f"(dep_f) : "r"(md0));
         if (TRACK) dh00 += (md0 != 0u && idx == origin_idx) ? 2 : 0;
     } else if (MODE == 1) {
-        // both probabilities > 0: 32-bit inclusive thresholds.  A site is a minimum or a maximum, never both: the
-        // threshold is chosen by the site type, one compare decides.
-        const bool is_min = md0 != 0u;
-        const bool ok = accept_word <= (is_min ? P.tp_incl : P.tq_incl);
-        const uint32_t m = ok ? (md0 | mr0) : 0u;
-        atomicXor(a, m);
-        n_dep += (ok && is_min) ? 1u : 0u;
-        n_rem += (m != 0u && !is_min) ? 1u : 0u;
-        if (TRACK) dh00 += (idx == origin_idx && m != 0u) ? (is_min ? 2 : -2) : 0;
+        // both probabilities > 0: 32-bit inclusive thresholds.  The two accept decisions do not depend on the
+        // lattice, so they are taken off the dependent chain (loads -> tests -> XOR): the site bit is masked by
+        // each decision beforehand.  A site is never a minimum and a maximum at once: md and mr are disjoint.
+        const uint32_t bit_p = (accept_word <= P.tp_incl) ? bit : 0u;
+        const uint32_t bit_q = (accept_word <= P.tq_incl) ? bit : 0u;
+        const uint32_t md = lop3_and_not_not(bit_p, t1, t2);
+        const uint32_t mr = lop3_and_not_not(bit_q, u1, u2);
+        atomicXor(a, md | mr);
+        asm("{ .reg .pred p; setp.ne.u32 p, %1, 0; @p add.f32 %0, %0, 0f3F800000; }" : "+f"(dep_f) : "r"(md));
+        asm("{ .reg .pred p; setp.ne.u32 p, %1, 0; @p add.f32 %0, %0, 0f3F800000; }" : "+f"(rem_f) : "r"(mr));
+        if (TRACK) dh00 += (idx == origin_idx) ? (md ? 2 : (mr ? -2 : 0)) : 0;
     } else {
         // general thresholds (a probability of exactly 0 with the other one in (0,1])
-        const uint32_t md = ((uint64_t)accept_word < P.thr_p) ? md0 : 0u;
-        const uint32_t mr = ((uint64_t)accept_word < P.thr_q) ? mr0 : 0u;
+        const uint32_t md = ((uint64_t)accept_word < P.thr_p) ? lop3_and_not_not(bit, t1, t2) : 0u;
+        const uint32_t mr = ((uint64_t)accept_word < P.thr_q) ? lop3_and_not_not(bit, u1, u2) : 0u;
         atomicXor(a, md | mr);
         n_dep += (md != 0u) ? 1u : 0u;
         n_rem += (mr != 0u) ? 1u : 0u;
@@ -537,7 +548,7 @@ __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const 
     const uint32_t c_begin = WHOLE ? 0u : (SUBM == 2 ? (P.sub << 13) : P.call_begin);
     const uint32_t c_end = WHOLE ? (uint32_t)(T * T) / 8u : (SUBM == 2 ? c_begin + ((n_steps + 7u) >> 3) : P.call_end);
     uint4 cur, nxt, cur_a[2], nxt_a[2];
-    float dep_f = 0.0f;       // MODE 0: deposits of this tile (see attempt)
+    float dep_f = 0.0f, rem_f = 0.0f;       // MODE 0, 1: deposits / removals of this tile (see attempt)
     cur = philox4x32_10(c_begin, tile_id, P.m, replica, P.key);
     if (MODE) {
         cur_a[0] = philox4x32_10((2u * c_begin) | ACCEPT, tile_id, P.m, replica, P.key);
@@ -557,14 +568,14 @@ __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const 
         const uint32_t rem = n_steps - 8u * (c - c_begin);      // S7: live steps left in this call and after
         const uint4 a0 = MODE ? cur_a[0] : make_uint4(0u, 0u, 0u, 0u);
         const uint4 a1 = MODE ? cur_a[1] : make_uint4(0u, 0u, 0u, 0u);
-        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.x, a0.x, P, n_dep, dep_f, n_rem, dh00, origin_idx, SUBM != 2 || rem > 0u);
-        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.x * TT, a0.y, P, n_dep, dep_f, n_rem, dh00, origin_idx, SUBM != 2 || rem > 1u);
-        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.y, a0.z, P, n_dep, dep_f, n_rem, dh00, origin_idx, SUBM != 2 || rem > 2u);
-        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.y * TT, a0.w, P, n_dep, dep_f, n_rem, dh00, origin_idx, SUBM != 2 || rem > 3u);
-        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.z, a1.x, P, n_dep, dep_f, n_rem, dh00, origin_idx, SUBM != 2 || rem > 4u);
-        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.z * TT, a1.y, P, n_dep, dep_f, n_rem, dh00, origin_idx, SUBM != 2 || rem > 5u);
-        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.w, a1.z, P, n_dep, dep_f, n_rem, dh00, origin_idx, SUBM != 2 || rem > 6u);
-        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.w * TT, a1.w, P, n_dep, dep_f, n_rem, dh00, origin_idx, SUBM != 2 || rem > 7u);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.x, a0.x, P, n_dep, dep_f, n_rem, rem_f, dh00, origin_idx, SUBM != 2 || rem > 0u);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.x * TT, a0.y, P, n_dep, dep_f, n_rem, rem_f, dh00, origin_idx, SUBM != 2 || rem > 1u);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.y, a0.z, P, n_dep, dep_f, n_rem, rem_f, dh00, origin_idx, SUBM != 2 || rem > 2u);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.y * TT, a0.w, P, n_dep, dep_f, n_rem, rem_f, dh00, origin_idx, SUBM != 2 || rem > 3u);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.z, a1.x, P, n_dep, dep_f, n_rem, rem_f, dh00, origin_idx, SUBM != 2 || rem > 4u);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.z * TT, a1.y, P, n_dep, dep_f, n_rem, rem_f, dh00, origin_idx, SUBM != 2 || rem > 5u);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.w, a1.z, P, n_dep, dep_f, n_rem, rem_f, dh00, origin_idx, SUBM != 2 || rem > 6u);
+        attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.w * TT, a1.w, P, n_dep, dep_f, n_rem, rem_f, dh00, origin_idx, SUBM != 2 || rem > 7u);
         cur = nxt;
         if (MODE) {
             cur_a[0] = nxt_a[0];
@@ -572,6 +583,7 @@ __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const 
         }
     }
     n_dep += (uint32_t)dep_f;
+    n_rem += (uint32_t)rem_f;
 }
 
 // DEAD = false: one colour of schedule S4 per launch (P.slot);  DEAD = true: every tile of the dead-border schedule
