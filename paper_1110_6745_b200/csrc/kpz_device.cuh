@@ -160,6 +160,23 @@ __device__ __forceinline__ uint32_t enc_halo(uint32_t ly) {
     return ((ly >> 1) & 1u) | ((((y1 & 1u) ^ 1u) ^ ((y1 >> 1) & 1u)) << 31);
 }
 
+// N running pointers into consecutive rows of the bit-planes (periodic in y): one 64-bit add per pointer and row
+// instead of a multiply and a scaled add per access.
+template <int N>
+struct RowPtrs {
+    uint32_t* p[N];
+    uint32_t g;
+    __device__ __forceinline__ void next(uint32_t L, uint32_t W) {
+        ptrdiff_t st = (ptrdiff_t)W;
+        if (++g == L) {
+            g = 0u;
+            st -= (ptrdiff_t)L * (ptrdiff_t)W;
+        }
+#pragma unroll
+        for (int k = 0; k < N; ++k) p[k] += st;
+    }
+};
+
 // ---- a2: stage tile + halo, slopes (HBM) -> height bits (shared memory), T >= 32 -----------------------------
 template <int T, int NTHR, int NB = StageBatch<T>::N>
 __device__ __forceinline__ void stage_in_wide(const uint32_t* __restrict__ planeX, const uint32_t* __restrict__ planeY,
@@ -190,19 +207,23 @@ __device__ __forceinline__ void stage_in_wide(const uint32_t* __restrict__ plane
         }
     }
     uint32_t pendingH = 0u;    // halo word of the previous row: bit 0 already holds its +x halo
+    // words idx[0..WPL] of plane Y and words idx[0], idx[WPL] of plane X, row by row from y0
+    RowPtrs<WPL + 3> rp;
+    rp.g = y0;
+#pragma unroll
+    for (int k = 0; k <= WPL; ++k) rp.p[k] = const_cast<uint32_t*>(planeY) + (size_t)y0 * W + idx[k];
+    rp.p[WPL + 1] = const_cast<uint32_t*>(planeX) + (size_t)y0 * W + idx[0];
+    rp.p[WPL + 2] = const_cast<uint32_t*>(planeX) + (size_t)y0 * W + idx[WPL];
 #pragma unroll 1
     for (int l0 = 0; l0 <= T; l0 += NB) {
         uint32_t ry[NB][WPL + 1], rx[NB][2];
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
-            uint32_t g = y0 + (uint32_t)(l0 + b);
-            if (g >= L) g -= L;
-            const uint32_t* ly_ = planeY + (size_t)g * W;
-            const uint32_t* lx_ = planeX + (size_t)g * W;
 #pragma unroll
-            for (int k = 0; k <= WPL; ++k) ry[b][k] = ly_[idx[k]];
-            rx[b][0] = lx_[idx[0]];
-            rx[b][1] = lx_[idx[WPL]];
+            for (int k = 0; k <= WPL; ++k) ry[b][k] = *rp.p[k];
+            rx[b][0] = *rp.p[WPL + 1];
+            rx[b][1] = *rp.p[WPL + 2];
+            rp.next(L, W);
         }
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
@@ -258,28 +279,37 @@ __device__ __forceinline__ void stage_out_wide(uint32_t* __restrict__ planeX, ui
     idx[0] = x0 >> 5;
 #pragma unroll
     for (int k = 1; k <= WPL; ++k) idx[k] = (idx[k - 1] + 1u == W) ? 0u : idx[k - 1] + 1u;
+    // edge words (re-read) and all words (stored) of both planes, row by row from y0:
+    // ld: Y idx[0], Y idx[WPL], X idx[0], X idx[WPL];   st: Y idx[0..WPL], X idx[0..WPL]
+    RowPtrs<4> ld;
+    RowPtrs<2 * (WPL + 1)> st;
+    ld.g = st.g = y0;
+    ld.p[0] = planeY + (size_t)y0 * W + idx[0];
+    ld.p[1] = planeY + (size_t)y0 * W + idx[WPL];
+    ld.p[2] = planeX + (size_t)y0 * W + idx[0];
+    ld.p[3] = planeX + (size_t)y0 * W + idx[WPL];
+#pragma unroll
+    for (int k = 0; k <= WPL; ++k) {
+        st.p[k] = planeY + (size_t)y0 * W + idx[k];
+        st.p[WPL + 1 + k] = planeX + (size_t)y0 * W + idx[k];
+    }
 #pragma unroll 1
     for (int l0 = 0; l0 <= T; l0 += NB) {
         uint32_t ex[NB][2], ey[NB][2];
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
-            uint32_t g = y0 + (uint32_t)(l0 + b);
-            if (g >= L) g -= L;
-            const uint32_t* ly_ = planeY + (size_t)g * W;
-            const uint32_t* lx_ = planeX + (size_t)g * W;
-            ey[b][0] = ly_[idx[0]];
-            ey[b][1] = ly_[idx[WPL]];
-            ex[b][0] = lx_[idx[0]];
-            ex[b][1] = lx_[idx[WPL]];
+            ey[b][0] = *ld.p[0];
+            ey[b][1] = *ld.p[1];
+            ex[b][0] = *ld.p[2];
+            ex[b][1] = *ld.p[3];
+            ld.next(L, W);
         }
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
             const uint32_t ly = (uint32_t)(l0 + b);
             const uint32_t r = ly + 1u;
-            uint32_t g = y0 + ly;
-            if (g >= L) g -= L;
-            uint32_t* ly_ = planeY + (size_t)g * W;
-            uint32_t* lx_ = planeX + (size_t)g * W;
+            uint32_t* const* ly_ = st.p;               // *ly_[k] = word idx[k] of this row of plane Y
+            uint32_t* const* lx_ = st.p + (WPL + 1);   // ... of plane X
             uint32_t cur[WPL], below[WPL];
 #pragma unroll
             for (int k = 0; k < WPL; ++k) {
@@ -297,17 +327,17 @@ __device__ __forceinline__ void stage_out_wide(uint32_t* __restrict__ planeX, ui
                     // tile's own changed bits, atomically; rows 0..T-1 only
                     if (ly < (uint32_t)T) {
                         const uint32_t d0 = (ey[b][0] ^ (v[0] << s)) & ~lowmask;
-                        if (d0) atomicXor(ly_ + idx[0], d0);
+                        if (d0) atomicXor(ly_[0], d0);
 #pragma unroll
-                        for (int k = 1; k < WPL; ++k) ly_[idx[k]] = __funnelshift_l(v[k - 1], v[k], s);
+                        for (int k = 1; k < WPL; ++k) *ly_[k] = __funnelshift_l(v[k - 1], v[k], s);
                         const uint32_t d1 = (ey[b][1] ^ __funnelshift_l(v[WPL - 1], 0u, s)) & lowmask;
-                        if (d1) atomicXor(ly_ + idx[WPL], d1);
+                        if (d1) atomicXor(ly_[WPL], d1);
                     }
                 } else {
-                    ly_[idx[0]] = (ey[b][0] & lowmask) | (v[0] << s);
+                    *ly_[0] = (ey[b][0] & lowmask) | (v[0] << s);
 #pragma unroll
-                    for (int k = 1; k < WPL; ++k) ly_[idx[k]] = __funnelshift_l(v[k - 1], v[k], s);
-                    if (s != 0u) ly_[idx[WPL]] = (ey[b][1] & ~lowmask) | __funnelshift_l(v[WPL - 1], 0u, s);
+                    for (int k = 1; k < WPL; ++k) *ly_[k] = __funnelshift_l(v[k - 1], v[k], s);
+                    if (s != 0u) *ly_[WPL] = (ey[b][1] & ~lowmask) | __funnelshift_l(v[WPL - 1], 0u, s);
                 }
             }
             // sigma_x(.,ly): T+1 bits (lx = 0..T) at bit offset x0; rows 0..T-1 only
@@ -325,18 +355,19 @@ __device__ __forceinline__ void stage_out_wide(uint32_t* __restrict__ planeX, ui
                 if (DEAD) {
                     // S5: bits lx = 0..T-1 only (bit T is sigma_x of the right neighbour's own column 0)
                     const uint32_t d0 = (ex[b][0] ^ (v[0] << s)) & ~lowmask;
-                    if (d0) atomicXor(lx_ + idx[0], d0);
+                    if (d0) atomicXor(lx_[0], d0);
 #pragma unroll
-                    for (int k = 1; k < WPL; ++k) lx_[idx[k]] = __funnelshift_l(v[k - 1], v[k], s);
+                    for (int k = 1; k < WPL; ++k) *lx_[k] = __funnelshift_l(v[k - 1], v[k], s);
                     const uint32_t d1 = (ex[b][1] ^ __funnelshift_l(v[WPL - 1], 0u, s)) & lowmask;
-                    if (d1) atomicXor(lx_ + idx[WPL], d1);
+                    if (d1) atomicXor(lx_[WPL], d1);
                 } else {
-                    lx_[idx[0]] = (ex[b][0] & lowmask) | (v[0] << s);
+                    *lx_[0] = (ex[b][0] & lowmask) | (v[0] << s);
 #pragma unroll
-                    for (int k = 1; k < WPL; ++k) lx_[idx[k]] = __funnelshift_l(v[k - 1], v[k], s);
-                    lx_[idx[WPL]] = (ex[b][1] & ~lowmask1) | __funnelshift_l(v[WPL - 1], 0u, s) | (bitT << s);
+                    for (int k = 1; k < WPL; ++k) *lx_[k] = __funnelshift_l(v[k - 1], v[k], s);
+                    *lx_[WPL] = (ex[b][1] & ~lowmask1) | __funnelshift_l(v[WPL - 1], 0u, s) | (bitT << s);
                 }
             }
+            st.next(L, W);
         }
     }
 }
