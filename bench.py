@@ -40,7 +40,7 @@ ALG_ALU_OPS_PER_UPDATE = 11.5
 ALG_MUL_OPS_PER_UPDATE = 2.5
 ALG_BYTES_PER_UPDATE = 0.5          # each site (2 bits) read once and written once per MCS
 # dram__bytes_read.sum + dram__bytes_write.sum of one update launch at L = 2^17 (profiles/, ncu --set full)
-TRAFFIC_BYTES_PER_LAUNCH = 6.24e9
+TRAFFIC_BYTES_PER_LAUNCH = 6.27e9
 
 
 def _peaks():
