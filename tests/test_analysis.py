@@ -52,3 +52,11 @@ def test_config4_run_lengths_and_eq8_sampling_times():
     assert all(b > a for a, b in zip(t, t[1:]))
     # late times grow geometrically with ratio e^m
     assert t[-1] / t[-2] == pytest.approx(math.exp(0.01), rel=2e-3)
+
+
+def test_growth_sampling_times():
+    from paper_1110_6745_b200 import growth_run
+    assert growth_run.sampling_times(64) == [1, 2, 4, 5, 8, 10, 16, 20, 32, 50, 64]
+    ts = growth_run.sampling_times(10000)
+    assert ts[-1] == 10000 and all(t in ts for t in (1, 2, 5, 10, 20, 50, 100, 200, 500, 1000, 2000, 5000, 8192))
+    assert ts == sorted(set(ts))

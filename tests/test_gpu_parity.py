@@ -559,3 +559,24 @@ def test_poissonised_counts_parity(pkg, L, T, p, q, K, sched, seed):
     _compare_full(k, o)
     _compare_scalars(k, [o])
     assert k.counters()["attempts"] == a0 + L * L
+
+
+@pytest.mark.parametrize("L,T,p,q,seed,t_max", [(256, 16, 1.0, 0.0, 1, 64), (256, 64, 0.75, 0.25, 3, 20)])
+def test_growth_harness_against_oracle(pkg, L, T, p, q, seed, t_max):
+    """growth_run (config 1 in full: the {1,2,5}*10^n and 2^i times up to 64; a T = 64 general-(p,q) case): every
+    sample is the oracle's, bit for bit; beta_eff is eq. 11 applied to those samples; the invariant holds."""
+    import math
+    from paper_1110_6745_b200 import growth_run
+    out = growth_run.run(L, T, p, q, seed, t_max)
+    o = Oracle(L, p, q, T, seed, threads=NTHREADS)
+    o.init_flat()
+    t = 0
+    for row in out["samples"]:
+        o.run(row["t"] - t)
+        t = row["t"]
+        s1, s2, w2 = o.measure()
+        assert (row["sum_h"], row["sum_h2"], row["W2"]) == (s1, s2, w2)
+    assert out["invariant_sum_h"] and out["counters"]["attempts"] == t * L * L
+    w = {r["t"]: r["W2"] - 0.25 for r in out["samples"]}
+    for b in out["beta_eff"]:
+        assert b["beta_eff"] == 0.5 * math.log2(w[b["t"]] / w[b["t"] // 2])
