@@ -372,58 +372,83 @@ __device__ __forceinline__ void stage_out_wide(uint32_t* __restrict__ planeX, ui
     }
 }
 
-// ---- T < 32: a row is one word, bit p = lx+1.  nbits bits of a periodic bit-line starting at bit offset o
-// (a multiple of 4; the segment may span two words). -----------------------------------------------------------
-__device__ __forceinline__ uint32_t load_bits(const uint32_t* __restrict__ line, uint32_t W, uint32_t o, uint32_t mask) {
-    const uint32_t a = o >> 5;
-    const uint32_t a1 = (a + 1u == W) ? 0u : a + 1u;
-    return __funnelshift_r(line[a], line[a1], o) & mask;
-}
-
-// Writes the bits selected by `mask` (in segment coordinates) of `seg`.  Two same-colour tiles may share a
-// 32-bit word (and, for T = 4, a byte) when T < 32, so only the CHANGED bits are applied, with an XOR reduction:
-// every bit of a segment belongs to exactly one active tile, hence old ^ new on its own bits is exact.
-__device__ __forceinline__ void store_bits(uint32_t* __restrict__ line, uint32_t W, uint32_t o, uint32_t mask, uint32_t seg) {
-    const uint32_t a = o >> 5;
-    const uint32_t a1 = (a + 1u == W) ? 0u : a + 1u;
-    const uint32_t old = __funnelshift_r(line[a], line[a1], o) & mask;
-    const uint32_t d = old ^ (seg & mask);
-    const uint32_t s = o & 31u;
-    const uint32_t dlo = d << s;
-    const uint32_t dhi = __funnelshift_l(d, 0u, s);      // d >> (32 - s), 0 for s = 0
-    if (dlo) atomicXor(line + a, dlo);
-    if (dhi) atomicXor(line + a1, dhi);
-}
+// ---- T < 32: a row is one word, bit p = lx+1. -------------------------------------------------------------------
+// T < 32 staging: the rows of the tile are fetched (or re-read) in batches of up to 9 rows of two words per plane
+// before the first dependent use, so the global-memory latency is paid once per batch and not once per row.
+template <int T>
+struct NarrowBatch {
+    static constexpr int N = (T + 1 <= 9) ? T + 1 : 9;
+};
 
 template <int T, int NTHR>
 __device__ __forceinline__ void stage_in_narrow(const uint32_t* __restrict__ planeX, const uint32_t* __restrict__ planeY,
                                                 uint32_t L, uint32_t W, uint32_t x0, uint32_t y0, uint32_t* __restrict__ sm) {
     constexpr uint32_t MT = (1u << T) - 1u;          // T bits
     constexpr uint32_t MT1 = (2u << T) - 1u;         // T+1 bits
+    constexpr int R = T + 1, NB = NarrowBatch<T>::N;
+    const uint32_t a = x0 >> 5;
+    const uint32_t a1 = (a + 1u == W) ? 0u : a + 1u;
+    uint32_t g = y0;
+    size_t row = (size_t)y0 * W;
     uint32_t prev = 0u;                               // h1 of the previous row, bit lx
 #pragma unroll 1
-    for (uint32_t ly = 0; ly <= (uint32_t)T; ++ly) {
-        uint32_t g = y0 + ly;
-        if (g >= L) g -= L;
-        const uint32_t yv = load_bits(planeY + (size_t)g * W, W, x0, MT);
-        const uint32_t xv = load_bits(planeX + (size_t)g * W, W, x0, MT1);
-        const uint32_t yc = ycode(ly) & MT;
-        uint32_t cur;
-        if (ly == 0u) {
-            cur = prefix_xor32((xv ^ 0xAAAAAAAAu) & MT & ~1u) & MT;
-            sm[0] = ((cur ^ yv ^ yc) & MT) << 1;                       // row -1: own columns only
-        } else {
-            cur = prev ^ yv ^ yc;
+    for (int r0 = 0; r0 < R; r0 += NB) {
+        uint32_t yl[NB], yh[NB], xl[NB], xh[NB];
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            if (r0 + b < R) {
+                yl[b] = planeY[row + a];
+                yh[b] = planeY[row + a1];
+                if (r0 + b < T) {
+                    xl[b] = planeX[row + a];
+                    xh[b] = planeX[row + a1];
+                }
+                row += W;
+                if (++g == L) { g = 0u; row = 0; }
+            }
         }
-        uint32_t word = cur << 1;
-        if (ly < (uint32_t)T) {
-            const uint32_t hL = (cur ^ xv ^ ly) & 1u;
-            const uint32_t hR = ((cur >> (T - 1)) ^ (xv >> T) ^ ly) & 1u;
-            word |= hL | (hR << (T + 1));
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            const int r = r0 + b;
+            if (r < R) {
+                const uint32_t ly = (uint32_t)r;
+                const uint32_t yv = __funnelshift_r(yl[b], yh[b], x0) & MT;
+                const uint32_t xv = (r < T) ? (__funnelshift_r(xl[b], xh[b], x0) & MT1) : 0u;
+                const uint32_t yc = ycode(ly) & MT;
+                uint32_t cur;
+                if (r == 0) {
+                    cur = prefix_xor32((xv ^ 0xAAAAAAAAu) & MT & ~1u) & MT;
+                    sm[0] = ((cur ^ yv ^ yc) & MT) << 1;                       // row -1: own columns only
+                } else {
+                    cur = prev ^ yv ^ yc;
+                }
+                uint32_t word = cur << 1;
+                if (r < T) {
+                    const uint32_t hL = (cur ^ xv ^ ly) & 1u;
+                    const uint32_t hR = ((cur >> (T - 1)) ^ (xv >> T) ^ ly) & 1u;
+                    word |= hL | (hR << (T + 1));
+                }
+                sm[(ly + 1u) * NTHR] = word;
+                prev = cur;
+            }
         }
-        sm[(ly + 1u) * NTHR] = word;
-        prev = cur;
     }
+}
+
+// Writes the bits selected by `mask` (in segment coordinates) of `seg`; the segment sits at bit offset o (a multiple
+// of 4, it may span two words) and its two words were read before as (lo, hi).  Two same-colour tiles may share a
+// 32-bit word (and, for T = 4, a byte) when T < 32, so only the CHANGED bits are applied, with an XOR reduction:
+// every bit of a segment belongs to exactly one active tile, hence old ^ new on its own bits is exact (and stays so
+// when the words were read before other tiles' reductions landed).
+__device__ __forceinline__ void store_bits_pre(uint32_t* __restrict__ plo, uint32_t* __restrict__ phi, uint32_t o, uint32_t mask,
+                                               uint32_t seg, uint32_t lo, uint32_t hi) {
+    const uint32_t old = __funnelshift_r(lo, hi, o) & mask;
+    const uint32_t d = old ^ (seg & mask);
+    const uint32_t s = o & 31u;
+    const uint32_t dlo = d << s;
+    const uint32_t dhi = __funnelshift_l(d, 0u, s);      // d >> (32 - s), 0 for s = 0
+    if (dlo) atomicXor(plo, dlo);
+    if (dhi) atomicXor(phi, dhi);
 }
 
 template <int T, int NTHR, bool DEAD>
@@ -431,17 +456,43 @@ __device__ __forceinline__ void stage_out_narrow(uint32_t* __restrict__ planeX, 
                                                  uint32_t W, uint32_t x0, uint32_t y0, const uint32_t* __restrict__ sm) {
     constexpr uint32_t MT = (1u << T) - 1u;
     constexpr uint32_t MT1 = (2u << T) - 1u;
+    constexpr int R = DEAD ? T : T + 1;               // S5: the +y halo row belongs to the (active) tile above
+    constexpr int NB = NarrowBatch<T>::N;
+    const uint32_t a = x0 >> 5;
+    const uint32_t a1 = (a + 1u == W) ? 0u : a + 1u;
+    uint32_t g = y0, g2 = y0;
+    size_t row = (size_t)y0 * W, row2 = row;
 #pragma unroll 1
-    for (uint32_t ly = 0; ly <= (uint32_t)T; ++ly) {
-        uint32_t g = y0 + ly;
-        if (g >= L) g -= L;
-        const uint32_t word = sm[(ly + 1u) * NTHR], below = sm[ly * NTHR];
-        if (DEAD && ly == (uint32_t)T) break;      // S5: the +y halo row belongs to the (active) tile above
-        const uint32_t sy = ((word ^ below) >> 1) ^ ycode(ly);
-        store_bits(planeY + (size_t)g * W, W, x0, MT, sy);
-        if (ly < (uint32_t)T) {
-            const uint32_t sx = ((word ^ (word << 1)) >> 1) ^ ycode(ly);   // bit lx = h1(lx)^h1(lx-1)^h0(lx,ly), lx = 0..T
-            store_bits(planeX + (size_t)g * W, W, x0, DEAD ? MT : MT1, sx);   // S5: bit T belongs to the right tile
+    for (int r0 = 0; r0 < R; r0 += NB) {
+        uint32_t yl[NB], yh[NB], xl[NB], xh[NB];
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            if (r0 + b < R) {
+                yl[b] = planeY[row + a];
+                yh[b] = planeY[row + a1];
+                if (r0 + b < T) {
+                    xl[b] = planeX[row + a];
+                    xh[b] = planeX[row + a1];
+                }
+                row += W;
+                if (++g == L) { g = 0u; row = 0; }
+            }
+        }
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            const int r = r0 + b;
+            if (r < R) {
+                const uint32_t ly = (uint32_t)r;
+                const uint32_t word = sm[(ly + 1u) * NTHR], below = sm[ly * NTHR];
+                const uint32_t sy = ((word ^ below) >> 1) ^ ycode(ly);
+                store_bits_pre(planeY + row2 + a, planeY + row2 + a1, x0, MT, sy, yl[b], yh[b]);
+                if (r < T) {
+                    const uint32_t sx = ((word ^ (word << 1)) >> 1) ^ ycode(ly);   // bit lx = h1(lx)^h1(lx-1)^h0(lx,ly), lx = 0..T
+                    store_bits_pre(planeX + row2 + a, planeX + row2 + a1, x0, DEAD ? MT : MT1, sx, xl[b], xh[b]);   // S5: bit T belongs to the right tile
+                }
+                row2 += W;
+                if (++g2 == L) { g2 = 0u; row2 = 0; }
+            }
         }
     }
 }
