@@ -107,6 +107,7 @@ __device__ __forceinline__ void global_draw(const UpdateParams& P, uint32_t sub,
 //     local minimum at a site with parity pi  <=>  all four neighbours have h1 == own_h1 ^ pi,
 //     local maximum                           <=>  all four neighbours have h1 != own_h1 ^ pi,
 //     a flip in either direction              <=>  XOR of the site's own h1 bit  (one shared-memory reduction).
+// What is stored is u = h1 ^ E(x,y) (enc_word / enc_narrow below), which makes the two tests independent of pi.
 // Rows ly = -1 .. T (row index r = ly+1) hold the tile plus its 1-site halo on all four sides (the -x / -y
 // halos carry sigma_x(x0,.) / sigma_y(.,y0), which belong to the tile's own sites; the +x / +y halos are the slopes
 // on the inactive neighbours that a border update changes).
@@ -155,6 +156,8 @@ __device__ __forceinline__ uint32_t prefix_xor32(uint32_t t) {
 __device__ __forceinline__ uint32_t enc_word(uint32_t ly) {
     return ((ly & 1u) ? 0x66666666u : 0xCCCCCCCCu) ^ (0u - ((ly >> 1) & 1u));
 }
+// T < 32 (bit p of a row word is column p - 1): the same pattern one bit up, E has period 4 in x
+__device__ __forceinline__ uint32_t enc_narrow(uint32_t ly) { return __funnelshift_l(enc_word(ly), enc_word(ly), 1); }
 __device__ __forceinline__ uint32_t enc_halo(uint32_t ly) {
     const uint32_t y1 = ly + 1u;
     return ((ly >> 1) & 1u) | ((((y1 & 1u) ^ 1u) ^ ((y1 >> 1) & 1u)) << 31);
@@ -385,6 +388,7 @@ __device__ __forceinline__ void stage_in_narrow(const uint32_t* __restrict__ pla
                                                 uint32_t L, uint32_t W, uint32_t x0, uint32_t y0, uint32_t* __restrict__ sm) {
     constexpr uint32_t MT = (1u << T) - 1u;          // T bits
     constexpr uint32_t MT1 = (2u << T) - 1u;         // T+1 bits
+    constexpr uint32_t MROW = (4u << T) - 1u;        // T+2 bits of a row word (halo, T columns, halo)
     constexpr int R = T + 1, NB = NarrowBatch<T>::N;
     const uint32_t a = x0 >> 5;
     const uint32_t a1 = (a + 1u == W) ? 0u : a + 1u;
@@ -418,7 +422,7 @@ __device__ __forceinline__ void stage_in_narrow(const uint32_t* __restrict__ pla
                 uint32_t cur;
                 if (r == 0) {
                     cur = prefix_xor32((xv ^ 0xAAAAAAAAu) & MT & ~1u) & MT;
-                    sm[0] = ((cur ^ yv ^ yc) & MT) << 1;                       // row -1: own columns only
+                    sm[0] = (((cur ^ yv ^ yc) & MT) << 1) ^ (enc_narrow(0xFFFFFFFFu) & MROW);   // row -1: own columns only
                 } else {
                     cur = prev ^ yv ^ yc;
                 }
@@ -428,7 +432,7 @@ __device__ __forceinline__ void stage_in_narrow(const uint32_t* __restrict__ pla
                     const uint32_t hR = ((cur >> (T - 1)) ^ (xv >> T) ^ ly) & 1u;
                     word |= hL | (hR << (T + 1));
                 }
-                sm[(ly + 1u) * NTHR] = word;
+                sm[(ly + 1u) * NTHR] = word ^ (enc_narrow(ly) & MROW);
                 prev = cur;
             }
         }
@@ -456,6 +460,7 @@ __device__ __forceinline__ void stage_out_narrow(uint32_t* __restrict__ planeX, 
                                                  uint32_t W, uint32_t x0, uint32_t y0, const uint32_t* __restrict__ sm) {
     constexpr uint32_t MT = (1u << T) - 1u;
     constexpr uint32_t MT1 = (2u << T) - 1u;
+    constexpr uint32_t MROW = (4u << T) - 1u;
     constexpr int R = DEAD ? T : T + 1;               // S5: the +y halo row belongs to the (active) tile above
     constexpr int NB = NarrowBatch<T>::N;
     const uint32_t a = x0 >> 5;
@@ -483,7 +488,8 @@ __device__ __forceinline__ void stage_out_narrow(uint32_t* __restrict__ planeX, 
             const int r = r0 + b;
             if (r < R) {
                 const uint32_t ly = (uint32_t)r;
-                const uint32_t word = sm[(ly + 1u) * NTHR], below = sm[ly * NTHR];
+                const uint32_t word = sm[(ly + 1u) * NTHR] ^ (enc_narrow(ly) & MROW);
+                const uint32_t below = sm[ly * NTHR] ^ (enc_narrow(ly - 1u) & MROW);
                 const uint32_t sy = ((word ^ below) >> 1) ^ ycode(ly);
                 store_bits_pre(planeY + row2 + a, planeY + row2 + a1, x0, MT, sy, yl[b], yh[b]);
                 if (r < T) {
@@ -502,21 +508,6 @@ __device__ __forceinline__ void stage_out_narrow(uint32_t* __restrict__ planeX, 
 // thread's tile holds global site (0,0) at local index origin_idx.  A flip is one shared-memory XOR reduction
 // (ATOMS.XOR without return) with a zero mask when nothing flips: no branch on the outcome, so a whole batch of
 // attempts stays one basic block for the instruction scheduler.
-__device__ __forceinline__ uint32_t lop3_any_differs(uint32_t v, uint32_t a, uint32_t b) {
-    uint32_t r;   // (v ^ a) | (v ^ b)
-    asm("lop3.b32 %0, %1, %2, %3, 0x7e;" : "=r"(r) : "r"(v), "r"(a), "r"(b));
-    return r;
-}
-__device__ __forceinline__ uint32_t lop3_all_differ(uint32_t v, uint32_t a, uint32_t b) {
-    uint32_t r;   // (v ^ a) & (v ^ b)
-    asm("lop3.b32 %0, %1, %2, %3, 0x18;" : "=r"(r) : "r"(v), "r"(a), "r"(b));
-    return r;
-}
-__device__ __forceinline__ uint32_t lop3_and3(uint32_t m, uint32_t x, uint32_t y) {
-    uint32_t r;   // m & x & y
-    asm("lop3.b32 %0, %1, %2, %3, 0x80;" : "=r"(r) : "r"(m), "r"(x), "r"(y));
-    return r;
-}
 __device__ __forceinline__ uint32_t lop3_and_not_not(uint32_t m, uint32_t x, uint32_t y) {
     uint32_t r;   // m & ~x & ~y
     asm("lop3.b32 %0, %1, %2, %3, 0x10;" : "=r"(r) : "r"(m), "r"(x), "r"(y));
@@ -562,25 +553,14 @@ __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site
         bit = edge ? 0u : bit;
     }
     bit = live ? bit : 0u;      // S7: steps beyond the tile's Poissonised count (constant true elsewhere)
-    // min_mask(b) / max_mask(b): b where the site is a local minimum / maximum, else 0
-    uint32_t t1, t2, u1 = 0u, u2 = 0u;
-    if constexpr (G::WIDE) {
-        // parity-free encoding (enc_word): minimum <=> right, up equal the site's bit and left, down differ
-        t1 = lop3<0xDB>(wo, wl, wr);      // (o^~l)|(o^r): not a minimum along x
-        t2 = lop3<0xBD>(wo, wu, wd);      // (o^u)|(o^~d): not a minimum along y
-        if (MODE != 0) {
-            u1 = lop3<0xBD>(wo, wl, wr);  // not a maximum along x
-            u2 = lop3<0xDB>(wo, wu, wd);  // not a maximum along y
-        }
-    } else {
-        // v: bit = own_h1 ^ pi at every position of the word (rotation of 0xAAAAAAAA by the row parity)
-        const uint32_t v = wo ^ __funnelshift_r(0xAAAAAAAAu, 0xAAAAAAAAu, ly + 1u);
-        t1 = lop3_any_differs(v, wl, wr);         // minimum <=> no neighbour differs from v
-        t2 = lop3_any_differs(v, wd, wu);
-        if (MODE != 0) {
-            u1 = ~lop3_all_differ(v, wl, wr);     // maximum <=> all four differ
-            u2 = ~lop3_all_differ(v, wd, wu);
-        }
+    // parity-free encoding (enc_word / enc_narrow): minimum <=> right, up equal the site's bit and left, down differ;
+    // t1, t2 (u1, u2): set where the site is NOT a minimum (maximum) along x, y
+    const uint32_t t1 = lop3<0xDB>(wo, wl, wr);      // (o^~l)|(o^r)
+    const uint32_t t2 = lop3<0xBD>(wo, wu, wd);      // (o^u)|(o^~d)
+    uint32_t u1 = 0u, u2 = 0u;
+    if (MODE != 0) {
+        u1 = lop3<0xBD>(wo, wl, wr);
+        u2 = lop3<0xDB>(wo, wu, wd);
     }
     if (MODE == 0) {
         const uint32_t md0 = lop3_and_not_not(bit, t1, t2);
