@@ -655,7 +655,9 @@ __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const 
 template <int T, int NTHR, int MODE, bool DEAD, int SUB>
 // T = 64: CTAs of 96 threads, three per SM = 9 warps (eight 32-thread CTAs are the limit otherwise: 1 KB of shared
 // memory is reserved per CTA); measured on B200 at L = 2^16: 690 against 681 Gupd/s
-__global__ void __launch_bounds__(NTHR, (T == 64) ? 3 : 1) kpz_update_kernel(const UpdateParams P) {
+// T = 32: 64-thread CTAs; asking for 8 per SM caps the registers at 125 (16 warps per SM: 834 against 790 Gupd/s at
+// L = 2^16; tighter caps spill and slow the small, chain-bound lattices of config 2)
+__global__ void __launch_bounds__(NTHR, (T == 64) ? 3 : (T == 32 ? 8 : 1)) kpz_update_kernel(const UpdateParams P) {
     using G = TileGeom<T>;
     extern __shared__ uint32_t smem[];
     uint32_t* sm = smem + threadIdx.x;
