@@ -4,6 +4,7 @@ beta_eff(t) = (1/2) log2[(W^2(t) - 1/4) / (W^2(t/2) - 1/4)] (eq. 11, P:97-105, t
 and the exact invariant sum_h(t) = L^2/2 + 2 (deposits - removals).  Everything heavy runs in the kernels.
 
     python -m paper_1110_6745_b200.growth_run --L 131072 --tile 64 --seed 42 --t-max 10000
+    python -m paper_1110_6745_b200.growth_run --L 524288 --tile 64 --p 0.75 --q 0.25 --seed 3 --t-max 50 --every
 """
 from __future__ import annotations
 
@@ -21,11 +22,11 @@ def sampling_times(t_max):
     return sorted(t for t in ts if t <= t_max)
 
 
-def run(L, tile, p=1.0, q=0.0, seed=42, t_max=10000, device="cuda:0"):
+def run(L, tile, p=1.0, q=0.0, seed=42, t_max=10000, device="cuda:0", every=False):
     k = KPZ(L, p, q, tile, seed, device=device)
     try:
         k.init_flat()
-        times = sampling_times(t_max)
+        times = list(range(1, t_max + 1)) if every else sampling_times(t_max)      # config 5: t = 1..50
         t0 = time.time()
         s1, s2, w2 = k.run_sampled(times)
         k.synchronize()
@@ -52,8 +53,9 @@ def main():
     ap.add_argument("--q", type=float, default=0.0)
     ap.add_argument("--seed", type=int, default=7)
     ap.add_argument("--t-max", type=int, default=1000)
+    ap.add_argument("--every", action="store_true", help="sample after every MCS (config 5) instead of the log-spaced times")
     a = ap.parse_args()
-    print(json.dumps(run(a.L, a.tile, a.p, a.q, a.seed, a.t_max)))
+    print(json.dumps(run(a.L, a.tile, a.p, a.q, a.seed, a.t_max, every=a.every)))
 
 
 if __name__ == "__main__":
