@@ -165,6 +165,25 @@ int32_t kpz_import_packed(kpz_ctx* ctx, const void* host_src, size_t bytes, cons
 int32_t kpz_step_host(kpz_ctx* ctx, void* host_lattice, size_t bytes, int64_t* h00_inout, uint64_t mcs_start,
                       uint64_t mcs, int64_t* sum_h, int64_t* sum_h2, double* W2);
 
+/* Pipelined end-to-end steps with HOST buffers: n_lanes independent lattices
+ * (same L, p, q, tile, seed as the handle; they differ in state and MCS clock), each a HOST buffer of `bytes` >=
+ * lattice_bytes in the device layout above (pinned memory is required for the copies to overlap), are each advanced
+ * by `mcs` MCS and measured, n_rounds times over, in the order round 0: lane 0 .. n_lanes-1, round 1: ... .  Each
+ * batch is exactly one kpz_step_host (same kernels, same results, bit for bit); what differs is the plumbing: the
+ * handle's bound lattice and `device_lattice2` (a second DEVICE buffer of lattice_bytes, 16-byte aligned, owned by
+ * the caller) alternate, the host->device copy of batch b+1 and the device->host copy of batch b-1 run on two
+ * internal non-blocking streams while the kernels of batch b run on the bound stream.
+ *   host_lattices : HOST array of n_lanes HOST pointers; each lattice is overwritten with its advanced state
+ *   h00_inout     : HOST [n_lanes][n_replicas] tracked height of site (0,0), in and out (NULL = zeros, not returned)
+ *   mcs_start     : HOST [n_lanes] MCS clock of each lane on entry (lane clocks advance by mcs per round)
+ *   sum_h, sum_h2, W2 : HOST [n_rounds][n_lanes][n_replicas] out-arrays (any may be NULL), as kpz_measure
+ * Synchronises before returning.  Afterwards the handle's own lattice, counters and MCS clock are unspecified:
+ * call kpz_init_flat, kpz_set_slopes or kpz_import_packed before using it again.  KPZ_EINVAL for NULL / short /
+ * misaligned buffers, n_lanes = 0 or n_rounds = 0; KPZ_EOVERFLOW as kpz_measure (the run completes). */
+int32_t kpz_pipeline_host(kpz_ctx* ctx, void* device_lattice2, size_t device_lattice2_bytes, uint32_t n_lanes,
+                          void* const* host_lattices, size_t bytes, int64_t* h00_inout, const uint64_t* mcs_start,
+                          uint64_t mcs, uint32_t n_rounds, int64_t* sum_h, int64_t* sum_h2, double* W2);
+
 /* ---- power spectrum along the lattice axes (eq. 15-16) ---------------- */
 
 /* Exact integer profiles of replica `replica`: col_sums[x] = sum_y h(x,y), row_sums[y] = sum_x h(x,y) with absolute

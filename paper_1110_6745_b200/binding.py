@@ -20,7 +20,7 @@ _lib = None
 exported_symbols = [
     "kpz_workspace_bytes", "kpz_create", "kpz_create_batch", "kpz_bind", "kpz_init_flat", "kpz_run", "kpz_measure",
     "kpz_destroy", "kpz_synchronize", "kpz_last_error", "kpz_get_slopes", "kpz_get_window", "kpz_set_slopes",
-    "kpz_state_hash", "kpz_counters", "kpz_export_packed", "kpz_import_packed", "kpz_step_host",
+    "kpz_state_hash", "kpz_counters", "kpz_export_packed", "kpz_import_packed", "kpz_step_host", "kpz_pipeline_host",
     "kpz_launch_count", "kpz_philox_selftest", "kpz_profiles", "kpz_power_spectrum", "kpz_set_schedule", "kpz_set_sub_sweeps", "kpz_run_sampled", "kpz_set_poisson",
 ]
 
@@ -66,6 +66,7 @@ def load_library() -> ctypes.CDLL:
         "kpz_export_packed": [vp, vp, sz],
         "kpz_import_packed": [vp, vp, sz, vp, u64],
         "kpz_step_host": [vp, vp, sz, vp, u64, u64, vp, vp, vp],
+        "kpz_pipeline_host": [vp, vp, sz, u32, vp, sz, vp, vp, u64, u32, vp, vp, vp],
         "kpz_launch_count": [vp, vp],
         "kpz_philox_selftest": [vp, vp, vp, u32],
     }
@@ -234,6 +235,27 @@ class KPZ:
         w2 = np.zeros(R, dtype=np.float64)
         self._check(self._lib.kpz_step_host(self._h, host_tensor.data_ptr(), host_tensor.numel(), h00.ctypes.data,
                                             int(mcs_start), int(mcs), s1.ctypes.data, s2.ctypes.data, w2.ctypes.data))
+        return s1, s2, w2
+
+    def pipeline_host(self, host_tensors, h00, mcs_start, mcs, n_rounds=1):
+        """kpz_pipeline_host: every pinned host lattice of `host_tensors` advanced by mcs MCS and measured, n_rounds
+        times, copies overlapped with the kernels.  h00 (int64 [n_lanes, R]) is updated in place.  Returns sum_h,
+        sum_h2, W2 of shape [n_rounds, n_lanes, R]."""
+        torch = self._torch
+        R, n = self.n_replicas, len(host_tensors)
+        if getattr(self, "lattice2", None) is None:
+            with torch.cuda.device(self.device):
+                self.lattice2 = torch.empty(self.lattice_bytes, dtype=torch.uint8, device=self.device)
+        ptrs = (ctypes.c_void_p * n)(*[t.data_ptr() for t in host_tensors])
+        nbytes = min(t.numel() for t in host_tensors)
+        start = np.ascontiguousarray(mcs_start, dtype=np.uint64)
+        assert start.size == n and h00.dtype == np.int64 and h00.size == n * R and h00.flags.c_contiguous
+        s1 = np.zeros((n_rounds, n, R), dtype=np.int64)
+        s2 = np.zeros((n_rounds, n, R), dtype=np.int64)
+        w2 = np.zeros((n_rounds, n, R), dtype=np.float64)
+        self._check(self._lib.kpz_pipeline_host(self._h, self.lattice2.data_ptr(), self.lattice_bytes, n,
+                                                ctypes.addressof(ptrs), nbytes, h00.ctypes.data, start.ctypes.data,
+                                                int(mcs), int(n_rounds), s1.ctypes.data, s2.ctypes.data, w2.ctypes.data))
         return s1, s2, w2
 
     def launch_count(self):

@@ -589,6 +589,113 @@ int32_t kpz_step_host(kpz_ctx* c, void* host_lattice, size_t bytes, int64_t* h00
     return rc;
 }
 
+namespace {
+
+// streams and events of one kpz_pipeline_host call, released on every return path
+struct PipelineResources {
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    std::vector<cudaEvent_t> ev;
+    ~PipelineResources() {
+        for (cudaEvent_t e : ev) if (e) cudaEventDestroy(e);
+        if (s_in) cudaStreamDestroy(s_in);
+        if (s_out) cudaStreamDestroy(s_out);
+    }
+};
+
+// overwrite the tracked h(0,0) of every replica (stats[r][2]) and clear the S7 attempt counter, on the bound stream
+int32_t set_h00(kpz_ctx* c, const int64_t* h00) {
+    std::vector<unsigned long long> st((size_t)c->R * 4, 0ull);
+    KPZ_CUDA(c, cudaMemcpyAsync(st.data(), c->d_scratch + c->sl.stats, (size_t)c->R * 32, cudaMemcpyDeviceToHost, c->stream));
+    KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (uint32_t r = 0; r < c->R; ++r) { st[4 * r + 2] = (unsigned long long)(h00 ? h00[r] : 0); st[4 * r + 3] = 0ull; }
+    KPZ_CUDA(c, cudaMemcpyAsync(c->d_scratch + c->sl.stats, st.data(), (size_t)c->R * 32, cudaMemcpyHostToDevice, c->stream));
+    KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
+    return KPZ_OK;
+}
+
+}  // namespace
+
+int32_t kpz_pipeline_host(kpz_ctx* c, void* device_lattice2, size_t device_lattice2_bytes, uint32_t n_lanes,
+                          void* const* host_lattices, size_t bytes, int64_t* h00_inout, const uint64_t* mcs_start,
+                          uint64_t mcs, uint32_t n_rounds, int64_t* sum_h, int64_t* sum_h2, double* W2) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    if (!device_lattice2 || device_lattice2_bytes < c->lattice_bytes || ((uintptr_t)device_lattice2 & 15u))
+        return fail(c, KPZ_EINVAL, "second device lattice missing, too small or not 16-byte aligned");
+    if (n_lanes == 0 || n_rounds == 0 || !host_lattices || !mcs_start || bytes < c->lattice_bytes)
+        return fail(c, KPZ_EINVAL, "bad argument");
+    for (uint32_t l = 0; l < n_lanes; ++l) {
+        if (!host_lattices[l]) return fail(c, KPZ_EINVAL, "NULL host lattice");
+        if (mcs_start[l] + (uint64_t)n_rounds * mcs > 0xFFFFFFFFull) return fail(c, KPZ_EINVAL, "MCS clock would exceed 2^32-1");
+    }
+    const uint64_t B = (uint64_t)n_lanes * n_rounds;   // batches, b = round * n_lanes + lane
+    PipelineResources res;
+    KPZ_CUDA(c, cudaStreamCreateWithFlags(&res.s_in, cudaStreamNonBlocking));
+    KPZ_CUDA(c, cudaStreamCreateWithFlags(&res.s_out, cudaStreamNonBlocking));
+    res.ev.assign((size_t)B * 2, nullptr);               // per batch: copied in, copied out
+    for (cudaEvent_t& e : res.ev) KPZ_CUDA(c, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    uint32_t* const dbuf[2] = {c->d_lattice, static_cast<uint32_t*>(device_lattice2)};
+    std::vector<int64_t> h00((size_t)n_lanes * c->R, 0);
+    if (h00_inout) std::memcpy(h00.data(), h00_inout, h00.size() * sizeof(int64_t));
+    std::vector<uint64_t> clock(mcs_start, mcs_start + n_lanes);
+
+    // host->device copy of batch b: its device slot must have been copied out (batch b-2), and so must the last
+    // batch of the same lane (b - n_lanes), whose output is this batch's input
+    auto enqueue_in = [&](uint64_t b) -> int32_t {
+        if (b >= 2) KPZ_CUDA(c, cudaStreamWaitEvent(res.s_in, res.ev[2 * (b - 2) + 1], 0));
+        if (b >= n_lanes) KPZ_CUDA(c, cudaStreamWaitEvent(res.s_in, res.ev[2 * (b - n_lanes) + 1], 0));
+        KPZ_CUDA(c, cudaMemcpyAsync(dbuf[b & 1], host_lattices[b % n_lanes], c->lattice_bytes, cudaMemcpyHostToDevice, res.s_in));
+        KPZ_CUDA(c, cudaEventRecord(res.ev[2 * b], res.s_in));
+        return KPZ_OK;
+    };
+
+    // Order of the host calls in one iteration: every small copy of the bookkeeping (counters out, h(0,0) of the
+    // next batch in) is issued while both copy engines are idle, i.e. before the two 'lattice_bytes' copies that
+    // follow the kernels; a small copy queued behind one of those would stall the bound stream for its length.
+    int32_t worst = KPZ_OK;
+    auto body = [&]() -> int32_t {
+        int32_t r = set_h00(c, &h00[0]);
+        if (r != KPZ_OK) return r;
+        if ((r = enqueue_in(0)) != KPZ_OK) return r;
+        for (uint64_t b = 0; b < B; ++b) {
+            const uint32_t lane = (uint32_t)(b % n_lanes);
+            // with one lane the next input is this batch's output: nothing to overlap, copy in after copy out
+            if (n_lanes >= 2 && b + 1 < B && (r = enqueue_in(b + 1)) != KPZ_OK) return r;
+            c->d_lattice = dbuf[b & 1];
+            c->mcs = clock[lane];
+            c->attempts_base = clock[lane] * (uint64_t)c->L * c->L;
+            KPZ_CUDA(c, cudaStreamWaitEvent(c->stream, res.ev[2 * b], 0));
+            if ((r = kpz_run(c, mcs)) != KPZ_OK) return r;
+            const size_t o = (size_t)b * c->R;
+            r = kpz_measure(c, sum_h ? sum_h + o : nullptr, sum_h2 ? sum_h2 + o : nullptr, W2 ? W2 + o : nullptr);
+            if (r == KPZ_EOVERFLOW) worst = r;
+            else if (r != KPZ_OK) return r;
+            // kpz_measure synchronised the bound stream: the lattice of batch b is final
+            for (uint32_t rep = 0; rep < c->R; ++rep) {
+                int64_t h;
+                if ((r = kpz_counters(c, rep, nullptr, nullptr, nullptr, &h, nullptr)) != KPZ_OK) return r;
+                h00[(size_t)lane * c->R + rep] = h;
+            }
+            clock[lane] += mcs;
+            if (b + 1 < B && (r = set_h00(c, &h00[(size_t)((b + 1) % n_lanes) * c->R])) != KPZ_OK) return r;
+            KPZ_CUDA(c, cudaMemcpyAsync(host_lattices[lane], dbuf[b & 1], c->lattice_bytes, cudaMemcpyDeviceToHost, res.s_out));
+            KPZ_CUDA(c, cudaEventRecord(res.ev[2 * b + 1], res.s_out));
+            if (n_lanes == 1 && b + 1 < B && (r = enqueue_in(b + 1)) != KPZ_OK) return r;
+        }
+        KPZ_CUDA(c, cudaStreamSynchronize(res.s_out));
+        return KPZ_OK;
+    };
+    rc = body();
+    c->d_lattice = dbuf[0];
+    if (rc != KPZ_OK) {          // drain the copy streams before their buffers can go away
+        cudaStreamSynchronize(res.s_in);
+        cudaStreamSynchronize(res.s_out);
+        return rc;
+    }
+    if (h00_inout) std::memcpy(h00_inout, h00.data(), h00.size() * sizeof(int64_t));
+    return worst;
+}
+
 // profiles of replica `replica` relative to h00 on the device (scratch prof[2][L]) + spectra; shared by the two calls
 static int32_t run_profiles(kpz_ctx* c, uint32_t replica, bool with_fft, long long* h00_out) {
     const uint32_t L = c->L, W = L / 32;

@@ -580,3 +580,69 @@ def test_growth_harness_against_oracle(pkg, L, T, p, q, seed, t_max):
     w = {r["t"]: r["W2"] - 0.25 for r in out["samples"]}
     for b in out["beta_eff"]:
         assert b["beta_eff"] == 0.5 * math.log2(w[b["t"]] / w[b["t"] // 2])
+
+
+@pytest.mark.parametrize("L,T,p,q,R,lanes", [(256, 16, 1.0, 0.0, 1, 3), (512, 64, 0.75, 0.25, 1, 2),
+                                              (128, 16, 0.75, 0.25, 3, 3), (2048, 32, 0.75, 0.25, 1, 1),
+                                              (4096, 64, 1.0, 0.0, 1, 2)])
+def test_pipeline_host_matches_oracle(pkg, L, T, p, q, R, lanes):
+    """kpz_pipeline_host: 1-3 lanes at different MCS clocks, 3 rounds of 2 MCS through pinned HOST lattices with the
+    copies overlapped; every batch's sums, every lane's final lattice and h(0,0) against the oracle, bit-exact."""
+    import torch
+    seed, mcs, rounds = 11, 2, 3
+    k = pkg.KPZ(L, p, q, T, seed, n_replicas=R)
+    k.init_flat()
+    hosts, h00, start = [], np.zeros((lanes, R), dtype=np.int64), []
+    for lane in range(lanes):                     # lane j starts from the state after 2j+1 MCS
+        k.run(1 if lane == 0 else 2)
+        t = torch.empty(k.lattice_bytes, dtype=torch.uint8).pin_memory()
+        k.export_packed(t)
+        hosts.append(t)
+        start.append(2 * lane + 1)
+        h00[lane] = [k.counters(r)["h00"] for r in range(R)]
+    s1, s2, w2 = k.pipeline_host(hosts, h00, start, mcs, rounds)
+    chk = pkg.KPZ(L, p, q, T, seed, n_replicas=R)
+    for r in range(R):
+        o = Oracle(L, p, q, T, seed, replica=r, threads=NTHREADS)
+        o.init_flat()
+        done = 0
+        want = {}
+        for t_end in sorted({start[lane] + mcs * (rd + 1) for lane in range(lanes) for rd in range(rounds)}):
+            o.run(t_end - done)
+            done = t_end
+            want[t_end] = (o.measure(), o.state_hash(), o.counters()["h00"])
+        for lane in range(lanes):
+            for rd in range(rounds):
+                t_end = start[lane] + mcs * (rd + 1)
+                assert (int(s1[rd, lane, r]), int(s2[rd, lane, r]), float(w2[rd, lane, r])) == want[t_end][0]
+            t_end = start[lane] + mcs * rounds
+            chk.import_packed(hosts[lane], h00[lane], t_end)
+            assert chk.state_hash(r) == want[t_end][1]
+            assert int(h00[lane, r]) == want[t_end][2]
+    # the handle works again after a re-import, and continues the trajectory of lane 0
+    k.import_packed(hosts[0], h00[0], start[0] + mcs * rounds)
+    k.run(1)
+    o = Oracle(L, p, q, T, seed, replica=0)
+    o.init_flat(); o.run(start[0] + mcs * rounds + 1)
+    assert k.state_hash(0) == o.state_hash()
+
+
+def test_pipeline_host_rejects_bad_arguments(pkg):
+    import ctypes
+    import torch
+    k = pkg.KPZ(64, 1.0, 0.0, 16, 1)
+    k.init_flat()
+    t = torch.empty(k.lattice_bytes, dtype=torch.uint8).pin_memory()
+    k.export_packed(t)
+    h00 = np.zeros((1, 1), dtype=np.int64)
+    with pytest.raises(pkg.KpzError):
+        k.pipeline_host([t], h00, [0], 1, 0)                         # no rounds
+    with pytest.raises(pkg.KpzError):
+        k.pipeline_host([t[:-1]], h00, [0], 1, 1)                    # host lattice too short
+    with pytest.raises(pkg.KpzError):
+        k.pipeline_host([t], h00, [0xFFFFFFFF], 1, 1)                # MCS clock overflow
+    k.init_flat()
+    k.run(1)                                                         # the handle is intact after a rejected call
+    o = Oracle(64, 1.0, 0.0, 16, 1)
+    o.init_flat(); o.run(1)
+    assert k.state_hash() == o.state_hash()
