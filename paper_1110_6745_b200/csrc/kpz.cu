@@ -613,6 +613,15 @@ int32_t set_h00(kpz_ctx* c, const int64_t* h00) {
     return KPZ_OK;
 }
 
+// tracked h(0,0) of every replica (stats[r][2]) in one copy on the bound stream
+int32_t get_h00(kpz_ctx* c, int64_t* h00) {
+    std::vector<unsigned long long> st((size_t)c->R * 4, 0ull);
+    KPZ_CUDA(c, cudaMemcpyAsync(st.data(), c->d_scratch + c->sl.stats, (size_t)c->R * 32, cudaMemcpyDeviceToHost, c->stream));
+    KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (uint32_t r = 0; r < c->R; ++r) h00[r] = (int64_t)st[4 * r + 2];
+    return KPZ_OK;
+}
+
 }  // namespace
 
 int32_t kpz_pipeline_host(kpz_ctx* c, void* device_lattice2, size_t device_lattice2_bytes, uint32_t n_lanes,
@@ -671,11 +680,7 @@ int32_t kpz_pipeline_host(kpz_ctx* c, void* device_lattice2, size_t device_latti
             if (r == KPZ_EOVERFLOW) worst = r;
             else if (r != KPZ_OK) return r;
             // kpz_measure synchronised the bound stream: the lattice of batch b is final
-            for (uint32_t rep = 0; rep < c->R; ++rep) {
-                int64_t h;
-                if ((r = kpz_counters(c, rep, nullptr, nullptr, nullptr, &h, nullptr)) != KPZ_OK) return r;
-                h00[(size_t)lane * c->R + rep] = h;
-            }
+            if ((r = get_h00(c, &h00[(size_t)lane * c->R])) != KPZ_OK) return r;
             clock[lane] += mcs;
             if (b + 1 < B && (r = set_h00(c, &h00[(size_t)((b + 1) % n_lanes) * c->R])) != KPZ_OK) return r;
             KPZ_CUDA(c, cudaMemcpyAsync(host_lattices[lane], dbuf[b & 1], c->lattice_bytes, cudaMemcpyDeviceToHost, res.s_out));
