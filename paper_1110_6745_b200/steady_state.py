@@ -4,6 +4,7 @@ the cumulants kappa_1..kappa_4 (eq. 18), the width distribution Psi_L(x) and the
 (eq. 15-16).  Everything heavy runs in the kernels; this file only drives them and applies analysis.py.
 
     python -m paper_1110_6745_b200.steady_state --L 128 --replicas 1024 [--t-end N] [--samples 100] [--tile 16]
+                                                  [--sub-sweeps K] [--spectrum-replicas 8] [--peaks]
 """
 from __future__ import annotations
 
@@ -16,11 +17,14 @@ from . import analysis
 from .binding import KPZ
 
 
-def run(L, replicas, tile=16, p=1.0, q=0.0, seed=4, t_end=None, samples=100, spectrum_replicas=8, device="cuda:0"):
+def run(L, replicas, tile=16, p=1.0, q=0.0, seed=4, t_end=None, samples=100, spectrum_replicas=8, device="cuda:0",
+        sub_sweeps=1):
     t_end = analysis.steady_state_t_end(L) if t_end is None else int(t_end)
     k = KPZ(L, p, q, tile, seed, n_replicas=replicas, device=device)
     try:
         k.init_flat()
+        if sub_sweeps > 1:
+            k.set_sub_sweeps(sub_sweeps)      # schedule S6
         t_half = t_end // 2
         k.run(t_half)
         step = max(1, (t_end - t_half) // max(1, samples))
@@ -34,6 +38,7 @@ def run(L, replicas, tile=16, p=1.0, q=0.0, seed=4, t_end=None, samples=100, spe
             k.run(t_end - t)
         w2 = np.array(w2) if w2 else k.measure()[2][None, :]
         out = {"L": L, "replicas": replicas, "tile": tile, "p": p, "q": q, "seed": seed, "t_end": t_end,
+               "sub_sweeps": sub_sweeps,
                "n_samples": int(w2.size), "cumulants": list(analysis.cumulants(w2)),
                "W2_final_mean": float(k.measure()[2].mean())}
         x, psi = analysis.width_distribution(w2)
@@ -48,6 +53,16 @@ def run(L, replicas, tile=16, p=1.0, q=0.0, seed=4, t_end=None, samples=100, spe
         k.close()
 
 
+def schedule_peaks(S, L, tile):
+    """S(k) at the mode numbers where the four-colour schedule leaves its imprint (odd multiples of L / (2 tile), and
+    L / 4), each beside the median of its 12 neighbouring modes (profiles/r01_config4_steady.md, addendum)."""
+    S = np.asarray(S)
+    n0 = L // (2 * tile)
+    modes = [n0 * j for j in range(5, tile, 2) if 6 <= n0 * j < len(S) - 6] + [L // 4]
+    return [{"n": n, "S": float(S[n]), "background": float(np.median(np.r_[S[n - 6:n], S[n + 1:n + 7]]))}
+            for n in modes]
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--L", type=int, default=128)
@@ -58,8 +73,16 @@ def main():
     ap.add_argument("--seed", type=int, default=4)
     ap.add_argument("--t-end", type=int, default=None, help="default: 20 L^1.61 (BASELINE config 4)")
     ap.add_argument("--samples", type=int, default=100)
+    ap.add_argument("--sub-sweeps", type=int, default=1, help="K sub-sweeps per MCS (schedule S6)")
+    ap.add_argument("--spectrum-replicas", type=int, default=8)
+    ap.add_argument("--peaks", action="store_true", help="print only S(k) at the schedule's peak modes")
     args = ap.parse_args()
-    print(json.dumps(run(args.L, args.replicas, args.tile, args.p, args.q, args.seed, args.t_end, args.samples)))
+    out = run(args.L, args.replicas, args.tile, args.p, args.q, args.seed, args.t_end, args.samples,
+              spectrum_replicas=args.spectrum_replicas, sub_sweeps=args.sub_sweeps)
+    if args.peaks:
+        out = {"L": out["L"], "tile": out["tile"], "replicas": out["spectrum_replicas"], "t_end": out["t_end"],
+               "sub_sweeps": out["sub_sweeps"], "peaks": schedule_peaks(out["S_k"], out["L"], out["tile"])}
+    print(json.dumps(out))
 
 
 if __name__ == "__main__":
