@@ -24,7 +24,10 @@
 // oracle/kpz_twin.py and by distribution tests): tile-colour order decode, offset draw, step -> Philox word map.
 //
 // Optional OpenMP: tiles of one colour are independent,
-// so the tile loop may run in parallel; results are identical for any thread count.
+// so the tile loop may run in parallel; results are identical for any thread count.  The same holds for the
+// loops over rows in kpzo_init_flat, over columns in kpzo_measure and over sites in kpzo_state_hash (exact
+// integer sums of independent terms): they are parallel too, so that the full-lattice parity cases at L = 2^16 and
+// 2^17 finish in minutes.  No arithmetic differs from the serial loops.
 
 #include <cstdint>
 #include <cstdlib>
@@ -370,9 +373,11 @@ int kpzo_get_threads(void* h) { return ((Oracle*)h)->nthreads; }
 // flat zig-zag start: h(x,y) = (x+y) mod 2 (W2 = 1/4; reading R7) => sx = sy = +1 if (x+y) odd else -1.
 void kpzo_init_flat(void* h) {
     Oracle* o = (Oracle*)h;
-    for (uint32_t ry = 0; ry < o->wh; ++ry)
+    // rows are independent: the loop over ry may run in parallel (plumbing only, same values)
+    #pragma omp parallel for schedule(static) num_threads(o->nthreads)
+    for (int64_t ry = 0; ry < (int64_t)o->wh; ++ry)
         for (uint32_t rx = 0; rx < o->ww; ++rx) {
-            uint32_t x = (o->wx0 + rx) % o->L, y = (o->wy0 + ry) % o->L;
+            uint32_t x = (o->wx0 + rx) % o->L, y = (o->wy0 + (uint32_t)ry) % o->L;
             int8_t v = ((x + y) & 1u) ? +1 : -1;
             o->sx[(size_t)ry * o->ww + rx] = v;
             o->sy[(size_t)ry * o->ww + rx] = v;
@@ -479,15 +484,29 @@ int kpzo_measure(void* h, uint64_t* sum_h_lohi, uint64_t* sum_h2_lohi, double* W
     if (!o->full) return -1;
     const uint32_t L = o->L;
     i128 S1 = 0, S2 = 0;
-    int64_t hx0 = o->h00;                       // h(0,0)
+    // walk along x on row 0 from the anchor h(0,0): h(x,0) = h(x-1,0) + sx(x,0)
+    std::vector<int64_t> row0(L);
+    int64_t hx0 = o->h00;
     for (uint32_t x = 0; x < L; ++x) {
-        if (x > 0) hx0 += o->sx[(size_t)0 * L + x];   // h(x,0) = h(x-1,0) + sx(x,0)
-        int64_t hh = hx0;
-        for (uint32_t y = 0; y < L; ++y) {
-            if (y > 0) hh += o->sy[(size_t)y * L + x];   // h(x,y) = h(x,y-1) + sy(x,y)
-            S1 += hh;
-            S2 += (i128)hh * hh;
+        if (x > 0) hx0 += o->sx[(size_t)0 * L + x];
+        row0[x] = hx0;
+    }
+    // then along y in every column x.  The columns are independent and the sums are exact integers, so the
+    // column loop may run in parallel (plumbing only: the same additions in another order).
+    #pragma omp parallel num_threads(o->nthreads)
+    {
+        i128 s1 = 0, s2 = 0;
+        #pragma omp for schedule(static) nowait
+        for (int64_t x = 0; x < (int64_t)L; ++x) {
+            int64_t hh = row0[(size_t)x];
+            for (uint32_t y = 0; y < L; ++y) {
+                if (y > 0) hh += o->sy[(size_t)y * L + (size_t)x];   // h(x,y) = h(x,y-1) + sy(x,y)
+                s1 += hh;
+                s2 += (i128)hh * hh;
+            }
         }
+        #pragma omp critical
+        { S1 += s1; S2 += s2; }
     }
     u128 N = (u128)L * L;
     i128 num = (i128)N * S2 - S1 * S1;
@@ -583,8 +602,9 @@ static inline uint64_t mix64(uint64_t z) {
 }
 uint64_t kpzo_state_hash(void* h) {
     Oracle* o = (Oracle*)h;
-    uint64_t acc = 0;
-    for (size_t n = 0; n < o->sx.size(); ++n) {
+    uint64_t acc = 0;       // a sum mod 2^64: any order gives the same value
+    #pragma omp parallel for reduction(+ : acc) schedule(static) num_threads(o->nthreads)
+    for (int64_t n = 0; n < (int64_t)o->sx.size(); ++n) {
         if (o->sx[n] == 1) acc += mix64(2 * n);
         if (o->sy[n] == 1) acc += mix64(2 * n + 1);
     }
