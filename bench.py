@@ -106,6 +106,11 @@ def run_ours(args):
 
     from paper_1110_6745_b200 import shard
     rank, world, local = shard.rank_world()
+    if world != args.gpus:       # the reported n_gpus can never disagree with the request
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%d (launch with torchrun --nproc-per-node %d, or let "
+                         "bench.py start the ranks itself by leaving WORLD_SIZE unset)" % (args.gpus, world, args.gpus))
+    if torch.cuda.device_count() <= local:
+        raise SystemExit("bench.py: rank %d needs cuda:%d but only %d device(s) are visible" % (rank, local, torch.cuda.device_count()))
     dist = None
     if world > 1:
         import torch.distributed as dist
@@ -302,6 +307,37 @@ def run_reference(args):
     print(json.dumps(out))
 
 
+def relaunch_under_torchrun(args):
+    """`python bench.py --gpus N` with N > 1 and no torchrun environment: start the N ranks ourselves (one process
+    per GPU, the driver's own command line) and pass their output through.  Returns the exit code."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), str(Path(__file__).resolve())] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
+def launcher_selftest(args):
+    """Host logic of the multi-rank launch without any kernel (tests/test_shard_gloo.py): every rank joins a gloo
+    group, takes the barrier and the two reductions of shard.aggregate; rank 0 prints the world it saw."""
+    import torch.distributed as dist
+    from paper_1110_6745_b200 import shard
+    rank, world, _ = shard.rank_world()
+    if world != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%d" % (args.gpus, world))
+    if world > 1:
+        dist.init_process_group("gloo")
+        dist.barrier()
+    units, seconds, rate = shard.aggregate(100.0 * (rank + 1), 1.0 + rank)
+    if rank == 0:
+        print(json.dumps({"launcher_selftest": True, "n_gpus": world, "units": units, "seconds": seconds, "rate": rate,
+                          "seeds": [shard.rank_seed(WORKLOAD["seed"], r) for r in range(world)]}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -310,12 +346,18 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--L", type=int, default=0, help="override the lattice size (debugging only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--launcher-selftest", action="store_true", help="multi-rank launch + reductions only (gloo, no GPU)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
-    else:
-        run_ours(args)
+        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(relaunch_under_torchrun(args))
+    if args.launcher_selftest:
+        launcher_selftest(args)
+        return
+    run_ours(args)
 
 
 if __name__ == "__main__":

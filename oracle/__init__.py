@@ -72,6 +72,8 @@ def lib() -> ctypes.CDLL:
         L.kpzo_get_shadow.argtypes = [vp, vp]
         L.kpzo_counters.argtypes = [vp, vp, vp, vp, vp, vp]
         L.kpzo_global_draw.argtypes = [vp, u32, vp, vp, vp]
+        L.kpzo_set_clock.argtypes = [vp, u64]
+        L.kpzo_set_clock.restype = ci
         L.kpzo_state_hash.argtypes = [vp]
         L.kpzo_state_hash.restype = u64
         L.kpzo_philox4x32_10.argtypes = [vp, vp, vp]
@@ -201,6 +203,11 @@ class Oracle:
         lib().kpzo_counters(self._h, ctypes.addressof(a), ctypes.addressof(d), ctypes.addressof(r),
                             ctypes.addressof(h), ctypes.addressof(m))
         return {"attempts": a.value, "deposits": d.value, "removals": r.value, "h00": h.value, "mcs": m.value}
+
+    def set_clock(self, mcs):
+        """MCS clock := mcs (attempts := mcs * L*L); the lattice is untouched."""
+        if lib().kpzo_set_clock(self._h, int(mcs)) != 0:
+            raise ValueError("the MCS clock is a 32-bit counter word")
 
     def global_draw(self, m):
         ox, oy = ctypes.c_uint32(), ctypes.c_uint32()

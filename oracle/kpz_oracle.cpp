@@ -422,7 +422,7 @@ uint32_t kpzo_poisson_table(void* h, uint32_t* kmin, uint64_t* thr) {
 int kpzo_run(void* h, uint64_t n_mcs) {
     Oracle* o = (Oracle*)h;
     for (uint64_t i = 0; i < n_mcs; ++i) {
-        if (o->mcs > 0xFFFFFFFFull) return -1;
+        if (o->mcs >= 0xFFFFFFFFull) return -1;     // the clock is a 32-bit counter word; 2^32 - 1 MCS at most
         run_one_mcs(o);
     }
     return 0;
@@ -559,6 +559,17 @@ void kpzo_get_shadow(void* h, int32_t* out) {
 void kpzo_counters(void* h, uint64_t* attempts, uint64_t* deposits, uint64_t* removals, int64_t* h00, uint64_t* mcs) {
     Oracle* o = (Oracle*)h;
     *attempts = o->attempts; *deposits = o->deposits; *removals = o->removals; *h00 = o->h00; *mcs = o->mcs;
+}
+
+// Sets the MCS clock (Philox counter word c2 of the next MCS, S1) without touching the lattice: the
+// state is then "as if" mcs fixed-count MCS had been run (attempts = mcs * L*L).  For parity cases that start a
+// trajectory near the end of the 32-bit clock.  Returns 0, or -1 if mcs > 2^32 - 1.
+int kpzo_set_clock(void* h, uint64_t mcs) {
+    Oracle* o = (Oracle*)h;
+    if (mcs > 0xFFFFFFFFull) return -1;
+    o->mcs = mcs;
+    o->attempts = mcs * (uint64_t)o->L * o->L;
+    return 0;
 }
 
 void kpzo_global_draw(void* h, uint32_t m, uint32_t* ox, uint32_t* oy, uint32_t* perm) {

@@ -71,7 +71,7 @@ int32_t validate(uint32_t L, double p, double q, uint32_t T, uint32_t R) {
     if (!valid_tile(T)) return KPZ_EINVAL;
     if (L == 0 || L % (2 * T) != 0 || L % 32 != 0) return KPZ_EINVAL;
     if (!(p >= 0.0 && p <= 1.0) || !(q >= 0.0 && q <= 1.0)) return KPZ_EINVAL;
-    if (R == 0) return KPZ_EINVAL;
+    if (R == 0 || R > 65535u) return KPZ_EINVAL;   // replicas index gridDim.y / gridDim.z of the measurement kernels
     if (L > (1u << 20)) return KPZ_EINVAL;   // int32 heights / tile ids stay in range up to 2^20
     const uint64_t NT = L / T;
     if (NT * NT >= 0xFFFFFFFFull) return KPZ_EINVAL;   // tile_id must never equal the global-draw marker
@@ -103,7 +103,7 @@ struct kpz_ctx {
     bool bound;
     ScratchLayout sl;
     size_t lattice_bytes;
-    int max_smem_optin;
+    int device;              // ordinal of the device that holds the bound buffers (-1 before kpz_bind)
     char err[512];
 };
 
@@ -126,6 +126,22 @@ int32_t fail(kpz_ctx* c, int32_t code, const char* fmt, ...) {
             return fail((c), KPZ_ECUDA, "%s failed: %s", #expr, cudaGetErrorString(e__));          \
     } while (0)
 
+// Makes the handle's device current for the duration of an entry point and restores the caller's device.
+struct DeviceGuard {
+    int prev = -1;
+    bool changed = false;
+    explicit DeviceGuard(int dev) {
+        if (dev >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != dev) changed = (cudaSetDevice(dev) == cudaSuccess);
+    }
+    ~DeviceGuard() {
+        if (changed) cudaSetDevice(prev);
+    }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
+constexpr int KPZ_MAX_DEVICES = 64;
+
 int grid_for(uint64_t n, int block, int cap = 148 * 16) {
     uint64_t g = (n + block - 1) / block;
     if (g > (uint64_t)cap) g = cap;
@@ -137,11 +153,13 @@ template <int T, int NTHR, int MODE, bool DEAD, int SUB>
 int32_t launch_update_k(kpz_ctx* c, const kpz::UpdateParams& P) {
     const size_t smem = (size_t)kpz::TileGeom<T>::WORDS * NTHR * sizeof(uint32_t);
     auto kern = kpz::kpz_update_kernel<T, NTHR, MODE, DEAD, SUB>;
-    static bool attr_set = false;
-    if (!attr_set) {
+    // function attributes are per device: one flag per device ordinal and instantiation
+    static bool attr_set[KPZ_MAX_DEVICES] = {};
+    const int dev = (c->device >= 0 && c->device < KPZ_MAX_DEVICES) ? c->device : 0;
+    if (!attr_set[dev]) {
         KPZ_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         KPZ_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-        attr_set = true;
+        attr_set[dev] = true;
     }
     const uint64_t blocks = (P.total_items + NTHR - 1) / NTHR;
     if (blocks > 0x7FFFFFFFull) return fail(c, KPZ_EINVAL, "too many tiles for one launch");
@@ -280,7 +298,7 @@ int32_t kpz_create_batch(kpz_ctx** out, uint32_t L, double p, double q, uint32_t
     c->L = L; c->T = tile; c->R = n_replicas; c->p = p; c->q = q; c->seed = seed;
     c->mcs = 0; c->launches = 0; c->schedule = KPZ_SCHEDULE_COLOURS; c->sub_sweeps = 1;
     c->poisson = false; c->pn = 0; c->pk_min = 0; c->attempts_base = 0;
-    c->d_lattice = nullptr; c->d_scratch = nullptr; c->stream = nullptr; c->bound = false;
+    c->d_lattice = nullptr; c->d_scratch = nullptr; c->stream = nullptr; c->bound = false; c->device = -1;
     c->sl = scratch_layout(L, n_replicas);
     c->lattice_bytes = (size_t)n_replicas * ((size_t)L * L / 4);
     c->err[0] = 0;
@@ -299,6 +317,15 @@ int32_t kpz_bind(kpz_ctx* c, void* d_lattice, size_t lattice_bytes, void* d_scra
     if (lattice_bytes < c->lattice_bytes || scratch_bytes < c->sl.total)
         return fail(c, KPZ_ENOMEM, "bound buffers too small: need %zu + %zu bytes", c->lattice_bytes, c->sl.total);
     if (((uintptr_t)d_lattice & 15u) || ((uintptr_t)d_scratch & 15u)) return fail(c, KPZ_EINVAL, "buffers must be 16-byte aligned");
+    // the device is the one that owns the buffers, whatever device is current in the calling thread
+    cudaPointerAttributes al, as;
+    KPZ_CUDA(c, cudaPointerGetAttributes(&al, d_lattice));
+    KPZ_CUDA(c, cudaPointerGetAttributes(&as, d_scratch));
+    if (al.type != cudaMemoryTypeDevice || as.type != cudaMemoryTypeDevice || al.device != as.device)
+        return fail(c, KPZ_EINVAL, "lattice and scratch must be device memory of one device");
+    if (al.device < 0 || al.device >= KPZ_MAX_DEVICES) return fail(c, KPZ_EINVAL, "device ordinal out of range");
+    c->device = al.device;
+    DeviceGuard dg__(c->device);
     c->d_lattice = static_cast<uint32_t*>(d_lattice);
     c->d_scratch = static_cast<unsigned char*>(d_scratch);
     c->stream = static_cast<cudaStream_t>(cuda_stream);
@@ -310,6 +337,7 @@ int32_t kpz_bind(kpz_ctx* c, void* d_lattice, size_t lattice_bytes, void* d_scra
 int32_t kpz_init_flat(kpz_ctx* c) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
     const uint64_t n_words = (uint64_t)c->R * ((uint64_t)c->L * c->L / 16);
     kpz::kpz_fill_flat_kernel<<<grid_for(n_words, 256, 148 * 32), 256, 0, c->stream>>>(c->d_lattice, n_words, c->L / 32);
     KPZ_CUDA(c, cudaGetLastError());
@@ -323,6 +351,7 @@ int32_t kpz_init_flat(kpz_ctx* c) {
 int32_t kpz_run(kpz_ctx* c, uint64_t mcs) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
     if (c->mcs + mcs > 0xFFFFFFFFull) return fail(c, KPZ_EINVAL, "MCS clock would exceed 2^32-1");
     for (uint64_t k = 0; k < mcs; ++k) {
         const uint32_t m = (uint32_t)c->mcs;
@@ -353,6 +382,7 @@ int32_t kpz_set_sub_sweeps(kpz_ctx* c, uint32_t K) {
     const uint32_t calls = c->T * c->T / 8u;
     if (K < 1 || K > calls || calls % K != 0) return fail(c, KPZ_EINVAL, "sub-sweeps must divide tile*tile/8");
     c->sub_sweeps = K;
+    DeviceGuard dg__(c->device);
     return (c->poisson && c->bound) ? upload_poisson_table(c) : KPZ_OK;
 }
 
@@ -386,6 +416,7 @@ static int32_t upload_poisson_table(kpz_ctx* c) {
 int32_t kpz_set_poisson(kpz_ctx* c, int32_t on) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
     c->poisson = on != 0;
     return c->poisson ? upload_poisson_table(c) : KPZ_OK;
 }
@@ -393,6 +424,7 @@ int32_t kpz_set_poisson(kpz_ctx* c, int32_t on) {
 int32_t kpz_measure(kpz_ctx* c, int64_t* sum_h, int64_t* sum_h2, double* W2) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
     std::vector<i128> S1, S2;
     std::vector<long long> h00;
     rc = measure_relative(c, S1, S2, h00);
@@ -417,6 +449,7 @@ int32_t kpz_measure(kpz_ctx* c, int64_t* sum_h, int64_t* sum_h2, double* W2) {
 int32_t kpz_run_sampled(kpz_ctx* c, const uint64_t* times, uint32_t n_times, int64_t* sum_h, int64_t* sum_h2, double* W2) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
     if (!times || n_times == 0) return fail(c, KPZ_EINVAL, "no sampling times");
     uint64_t prev = c->mcs;
     for (uint32_t i = 0; i < n_times; ++i) {
@@ -443,6 +476,7 @@ int32_t kpz_destroy(kpz_ctx* c) {
 int32_t kpz_synchronize(kpz_ctx* c) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
     KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
     return KPZ_OK;
 }
@@ -453,6 +487,7 @@ int32_t kpz_get_window(kpz_ctx* c, uint32_t replica, uint32_t x0, uint32_t y0, u
                        int8_t* sy) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
     if (replica >= c->R || !sx || !sy || w == 0 || h == 0 || w > c->L || h > c->L) return fail(c, KPZ_EINVAL, "bad window");
     const size_t n = (size_t)w * h;
     int8_t* d = nullptr;
@@ -477,6 +512,7 @@ int32_t kpz_get_slopes(kpz_ctx* c, uint32_t replica, int8_t* sx, int8_t* sy) {
 int32_t kpz_set_slopes(kpz_ctx* c, uint32_t replica, const int8_t* sx, const int8_t* sy, int64_t h00) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
     if (replica >= c->R || !sx || !sy) return fail(c, KPZ_EINVAL, "bad argument");
     const size_t n = (size_t)c->L * c->L;
     int8_t* d = nullptr;
@@ -513,6 +549,7 @@ int32_t kpz_set_slopes(kpz_ctx* c, uint32_t replica, const int8_t* sx, const int
 int32_t kpz_state_hash(kpz_ctx* c, uint32_t replica, uint64_t* out) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
     if (replica >= c->R || !out) return fail(c, KPZ_EINVAL, "bad argument");
     unsigned long long* acc = reinterpret_cast<unsigned long long*>(c->d_scratch + c->sl.misc);
     const uint64_t plane_words = (uint64_t)c->L * c->L / 32;
@@ -531,6 +568,7 @@ int32_t kpz_counters(kpz_ctx* c, uint32_t replica, uint64_t* attempts, uint64_t*
                      int64_t* h00, uint64_t* mcs) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
     if (replica >= c->R) return fail(c, KPZ_EINVAL, "replica out of range");
     unsigned long long st[4];
     KPZ_CUDA(c, cudaMemcpyAsync(st, c->d_scratch + c->sl.stats + (size_t)replica * 32, 32, cudaMemcpyDeviceToHost, c->stream));
@@ -546,6 +584,7 @@ int32_t kpz_counters(kpz_ctx* c, uint32_t replica, uint64_t* attempts, uint64_t*
 int32_t kpz_export_packed(kpz_ctx* c, void* host_dst, size_t bytes) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
     if (!host_dst || bytes < c->lattice_bytes) return fail(c, KPZ_EINVAL, "host buffer too small");
     KPZ_CUDA(c, cudaMemcpyAsync(host_dst, c->d_lattice, c->lattice_bytes, cudaMemcpyDeviceToHost, c->stream));
     KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -555,6 +594,7 @@ int32_t kpz_export_packed(kpz_ctx* c, void* host_dst, size_t bytes) {
 int32_t kpz_import_packed(kpz_ctx* c, const void* host_src, size_t bytes, const int64_t* h00, uint64_t mcs) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
     if (!host_src || bytes < c->lattice_bytes || mcs > 0xFFFFFFFFull) return fail(c, KPZ_EINVAL, "bad argument");
     KPZ_CUDA(c, cudaMemcpyAsync(c->d_lattice, host_src, c->lattice_bytes, cudaMemcpyHostToDevice, c->stream));
     std::vector<unsigned long long> st((size_t)c->R * 4, 0ull);
@@ -629,6 +669,7 @@ int32_t kpz_pipeline_host(kpz_ctx* c, void* device_lattice2, size_t device_latti
                           uint64_t mcs, uint32_t n_rounds, int64_t* sum_h, int64_t* sum_h2, double* W2) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
     if (!device_lattice2 || device_lattice2_bytes < c->lattice_bytes || ((uintptr_t)device_lattice2 & 15u))
         return fail(c, KPZ_EINVAL, "second device lattice missing, too small or not 16-byte aligned");
     if (n_lanes == 0 || n_rounds == 0 || !host_lattices || !mcs_start || bytes < c->lattice_bytes)
@@ -736,6 +777,7 @@ static int32_t run_profiles(kpz_ctx* c, uint32_t replica, bool with_fft, long lo
 int32_t kpz_profiles(kpz_ctx* c, uint32_t replica, int64_t* col_sums, int64_t* row_sums) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
     if (replica >= c->R) return fail(c, KPZ_EINVAL, "replica out of range");
     long long h00 = 0;
     rc = run_profiles(c, replica, false, &h00);
@@ -754,6 +796,7 @@ int32_t kpz_profiles(kpz_ctx* c, uint32_t replica, int64_t* col_sums, int64_t* r
 int32_t kpz_power_spectrum(kpz_ctx* c, uint32_t replica, double* S, double* Sx, double* Sy) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
     if (replica >= c->R) return fail(c, KPZ_EINVAL, "replica out of range");
     long long h00 = 0;
     rc = run_profiles(c, replica, true, &h00);

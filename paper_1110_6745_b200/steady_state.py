@@ -5,6 +5,8 @@ the cumulants kappa_1..kappa_4 (eq. 18), the width distribution Psi_L(x) and the
 
     python -m paper_1110_6745_b200.steady_state --L 128 --replicas 1024 [--t-end N] [--samples 100] [--tile 16]
                                                   [--sub-sweeps K] [--spectrum-replicas 8] [--peaks]
+    python -m paper_1110_6745_b200.steady_state --sizes 128,256,512,1024 --replicas 1024,256,256,256
+        (finite-size scaling over several sizes: alpha_eff(L) of eq. 13, the power laws of eq. 19 for kappa_1..kappa_4)
 """
 from __future__ import annotations
 
@@ -53,6 +55,29 @@ def run(L, replicas, tile=16, p=1.0, q=0.0, seed=4, t_end=None, samples=100, spe
         k.close()
 
 
+def finite_size_scaling(results):
+    """Finite-size scaling of a list of run() outputs of different L: alpha_eff(L) of eq. (13)
+    between sizes L and L/2 from kappa_1 = <W^2> -- with the intrinsic 1/4 of the zig-zag start subtracted and
+    without --, the power-law exponents of eq. (19) as alpha_n = s_n / (2 n) for the cumulants that are positive at
+    every size, and the fit of eq. (14) when at least three local slopes exist."""
+    results = sorted(results, key=lambda r: r["L"])
+    sizes = [r["L"] for r in results]
+    k1 = [r["cumulants"][0] for r in results]
+    out = {"sizes": sizes, "W2_mean": k1,
+           "alpha_eff": [{"L": L, "alpha_eff": a} for L, a in analysis.alpha_eff(sizes, k1)],
+           "alpha_eff_raw": [{"L": L, "alpha_eff": a} for L, a in analysis.alpha_eff(sizes, k1, intrinsic=0.0)],
+           "cumulant_power_laws": []}
+    for n in range(1, 5):
+        kn = [r["cumulants"][n - 1] for r in results]
+        if len(sizes) >= 2 and all(v > 0 for v in kn):
+            c, sl = analysis.fit_power_law(sizes, kn)
+            out["cumulant_power_laws"].append({"n": n, "prefactor": c, "exponent": sl, "alpha_n": sl / (2 * n)})
+    if len(out["alpha_eff"]) >= 3:
+        f = analysis.fit_correction([a["L"] for a in out["alpha_eff"]], [a["alpha_eff"] for a in out["alpha_eff"]])
+        out["eq14_fit"] = {"alpha": f["asymptote"], "a1": f["amplitude"], "omega1": f["exponent"], "rss": f["rss"]}
+    return out
+
+
 def schedule_peaks(S, L, tile):
     """S(k) at the mode numbers where the four-colour schedule leaves its imprint (odd multiples of L / (2 tile), and
     L / 4), each beside the median of its 12 neighbouring modes (profiles/r01_config4_steady.md, addendum)."""
@@ -66,7 +91,7 @@ def schedule_peaks(S, L, tile):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--L", type=int, default=128)
-    ap.add_argument("--replicas", type=int, default=1024)
+    ap.add_argument("--replicas", type=str, default="1024", help="replicas (one number, or one per entry of --sizes)")
     ap.add_argument("--tile", type=int, default=16)
     ap.add_argument("--p", type=float, default=1.0)
     ap.add_argument("--q", type=float, default=0.0)
@@ -76,7 +101,20 @@ def main():
     ap.add_argument("--sub-sweeps", type=int, default=1, help="K sub-sweeps per MCS (schedule S6)")
     ap.add_argument("--spectrum-replicas", type=int, default=8)
     ap.add_argument("--peaks", action="store_true", help="print only S(k) at the schedule's peak modes")
+    ap.add_argument("--sizes", type=str, default=None, help="comma-separated L: run every size, then finite_size_scaling")
     args = ap.parse_args()
+    if args.sizes:
+        sizes = [int(v) for v in args.sizes.split(",")]
+        reps = [int(v) for v in str(args.replicas).split(",")] if isinstance(args.replicas, str) else [args.replicas]
+        reps = reps * len(sizes) if len(reps) == 1 else reps
+        res = []
+        for L, R in zip(sizes, reps):
+            r = run(L, R, args.tile, args.p, args.q, args.seed, args.t_end, args.samples, spectrum_replicas=0,
+                    sub_sweeps=args.sub_sweeps)
+            res.append({k: r[k] for k in ("L", "replicas", "tile", "t_end", "n_samples", "cumulants", "W2_final_mean")})
+        print(json.dumps({"runs": res, "fss": finite_size_scaling(res)}))
+        return
+    args.replicas = int(args.replicas)
     out = run(args.L, args.replicas, args.tile, args.p, args.q, args.seed, args.t_end, args.samples,
               spectrum_replicas=args.spectrum_replicas, sub_sweeps=args.sub_sweeps)
     if args.peaks:

@@ -60,3 +60,82 @@ def test_growth_sampling_times():
     ts = growth_run.sampling_times(10000)
     assert ts[-1] == 10000 and all(t in ts for t in (1, 2, 5, 10, 20, 50, 100, 200, 500, 1000, 2000, 5000, 8192))
     assert ts == sorted(set(ts))
+
+
+def test_beta_eff_eq11_and_fit_eq12_recover_the_generating_parameters():
+    """eq. (9), (11), (12).  W(t) = b t^beta (1 + b1 t^phi1) with the paper's own numbers (beta = 0.2415,
+    b1 = -0.12, |phi1| = 1.05) on top of the intrinsic 1/4: the local slopes with t/t' = 2 tend to
+    beta, and the fit of the form (12) returns beta, b1, phi1.  The discrete slope of eq. (11) differs from the
+    derivative in eq. (12) by the known factor (2^-phi1 ... ) -- so the fit is pinned on the exact derivative, and the
+    discrete slopes on their own closed form."""
+    beta, b1, phi1, b = 0.2415, -0.12, -1.05, 0.7
+    t = np.array([2 ** i for i in range(4, 18)], dtype=np.float64)
+    W = b * t ** beta * (1.0 + b1 * t ** phi1)
+    be = analysis.beta_eff(t.astype(int), W ** 2 + 0.25)
+    assert [x[0] for x in be] == [int(v) for v in t[1:]]
+    for (tt, v) in be:
+        exact = beta + math.log2((1 + b1 * tt ** phi1) / (1 + b1 * (tt / 2) ** phi1))
+        assert v == pytest.approx(exact, abs=1e-12)
+    assert be[-1][1] == pytest.approx(beta, abs=2e-6)
+    # eq. (12) is the logarithmic derivative to first order in the correction: generate it exactly and refit
+    y = beta + b1 * phi1 * t ** phi1
+    f = analysis.fit_correction(t, y)
+    assert f["asymptote"] == pytest.approx(beta, abs=1e-9)
+    assert f["amplitude"] == pytest.approx(b1, rel=1e-6) and f["exponent"] == pytest.approx(phi1, rel=1e-6)
+    # with noise of the size of the paper's error bar (1.5e-3, P:105) beta is still recovered within it
+    rng = np.random.default_rng(12)
+    tt = np.array([50 * 1.3 ** i for i in range(28)])
+    f = analysis.fit_correction(tt, beta + b1 * phi1 * tt ** phi1 + rng.normal(0, 2e-4, tt.size))
+    assert f["asymptote"] == pytest.approx(beta, abs=1.5e-3)
+
+
+def test_alpha_eff_eq13_and_fit_eq14():
+    """eq. (10), (13), (14), P:119-127 with the paper's numbers (alpha = 0.393, a1 = -1.24, |omega1| = 1.16)."""
+    alpha, a1, om = 0.393, -1.24, -1.16
+    sizes = [2 ** i for i in range(7, 14)]
+    W = [0.4 * L ** alpha * (1 + a1 * L ** om) for L in sizes]
+    ae = analysis.alpha_eff(sizes, [w * w for w in W], intrinsic=0.0)
+    assert [x[0] for x in ae] == sizes[1:]
+    for L, v in ae:
+        assert v == pytest.approx(alpha + math.log2((1 + a1 * L ** om) / (1 + a1 * (L / 2) ** om)), abs=1e-12)
+    # pure power law: every local slope equals alpha; the intrinsic width is removed before the logarithm
+    ae = analysis.alpha_eff(sizes, [0.25 + 0.16 * L ** (2 * alpha) for L in sizes])
+    assert all(v == pytest.approx(alpha, abs=1e-12) for _, v in ae)
+    Ls = np.array(sizes, dtype=np.float64)
+    f = analysis.fit_correction(Ls, alpha + a1 * om * Ls ** om)
+    assert (f["asymptote"], f["amplitude"], f["exponent"]) == pytest.approx((alpha, a1, om), rel=1e-6)
+    with pytest.raises(ValueError):
+        analysis.fit_correction([1, 2], [1, 2])
+
+
+def test_cumulant_power_laws_eq19_eq20():
+    """eq. (19)-(20): kappa_n = L^(2 n alpha) (k0 + k1 L^-omega1)."""
+    alpha, om = 0.393, 1.16
+    sizes = np.array([512, 1024, 2048, 4096, 8192], dtype=np.float64)       # the sizes of Fig. 7
+    for n, (k0, k1) in enumerate([(0.05, 0.3), (2e-3, -0.01), (1e-4, 2e-3), (4e-6, 1e-4)], start=1):
+        pure = k0 * sizes ** (2 * n * alpha)
+        c, s = analysis.fit_power_law(sizes, pure)
+        assert c == pytest.approx(k0, rel=1e-9) and s / (2 * n) == pytest.approx(alpha, abs=1e-12)
+        kap = sizes ** (2 * n * alpha) * (k0 + k1 * sizes ** (-om))
+        f = analysis.fit_cumulant_fss(sizes, kap, n, alpha, omega1=om)
+        assert f["kappa0"] == pytest.approx(k0, rel=1e-8) and f["kappa1"] == pytest.approx(k1, rel=1e-6)
+        g = analysis.fit_cumulant_fss(sizes, kap, n, alpha)
+        assert g["omega1"] == pytest.approx(om, rel=1e-5) and g["kappa0"] == pytest.approx(k0, rel=1e-6)
+
+
+def test_finite_size_scaling_reduces_run_outputs():
+    """steady_state.finite_size_scaling on synthetic run() outputs: <W^2> = 1/4 + a L^(2 alpha) gives alpha_eff = alpha
+    at every size after the subtraction of the intrinsic width, and less without it (eq. 13); the cumulant power
+    laws of eq. (19) return alpha_n = alpha."""
+    from paper_1110_6745_b200 import steady_state
+    alpha = 0.393
+    runs = [{"L": L, "cumulants": [0.25 + 0.15 * L ** (2 * alpha), 2e-3 * L ** (4 * alpha), 1e-4 * L ** (6 * alpha),
+                                   -1.0]} for L in (128, 256, 512, 1024, 2048)]
+    f = steady_state.finite_size_scaling(runs)
+    assert [a["L"] for a in f["alpha_eff"]] == [256, 512, 1024, 2048]
+    assert all(a["alpha_eff"] == pytest.approx(alpha, abs=1e-12) for a in f["alpha_eff"])
+    assert all(a["alpha_eff"] < alpha for a in f["alpha_eff_raw"])
+    assert [c["n"] for c in f["cumulant_power_laws"]] == [1, 2, 3]    # kappa_4 < 0 here: no power law
+    assert all(c["alpha_n"] == pytest.approx(alpha, abs=1e-12) for c in f["cumulant_power_laws"][1:])
+    assert f["cumulant_power_laws"][0]["alpha_n"] < alpha               # kappa_1 still carries the additive 1/4
+    assert "eq14_fit" in f

@@ -258,38 +258,191 @@ def test_run_split_checkpoint_and_step_host(pkg):
     assert torch.equal(host, host2)                 # step_host wrote the advanced lattice back
 
 
-def _window_check(pkg, k, L, T, p, q, seed, n_mcs, wx0, wy0, W, check_h00=False):
-    M = 4 * (T + 1) * n_mcs
-    full = W + 2 * M
-    o = Oracle(L, p, q, T, seed, window=((wx0 - M) % L, (wy0 - M) % L, full, full), threads=NTHREADS)
-    o.init_flat(); o.run(n_mcs)
-    osx, osy = o.slopes()
-    gx, gy = k.get_window(wx0, wy0, W, W)
-    assert np.array_equal(gx, osx[M:M + W, M:M + W]), (wx0, wy0)
-    assert np.array_equal(gy, osy[M:M + W, M:M + W]), (wx0, wy0)
-    if check_h00:
-        assert k.counters()["h00"] == o.counters()["h00"]
+def _host_ram_gib():
+    for line in open("/proc/meminfo"):
+        if line.startswith("MemAvailable:"):
+            return int(line.split()[1]) / 2**20
+    return 0.0
+
+
+class _WindowSet:
+    """Light-cone window oracles (inner W x W exact for n_max MCS: margin M = 4 (T+1) n_max) advanced in
+    lockstep with the GPU lattice and compared at the sampled times."""
+
+    def __init__(self, L, T, p, q, seed, n_max, corners, W, schedule=None):
+        self.L, self.W, self.M = L, W, 4 * (T + 1) * n_max
+        full = W + 2 * self.M
+        self.items = []
+        for (wx0, wy0) in corners:
+            o = Oracle(L, p, q, T, seed, window=((wx0 - self.M) % L, (wy0 - self.M) % L, full, full), threads=NTHREADS)
+            if schedule:
+                o.set_schedule(schedule)
+            o.init_flat()
+            self.items.append((wx0 % L, wy0 % L, o))
+
+    def run(self, n):
+        for _, _, o in self.items:
+            o.run(n)
+
+    def check(self, k):
+        M, W = self.M, self.W
+        for wx0, wy0, o in self.items:
+            osx, osy = o.slopes()
+            gx, gy = k.get_window(wx0, wy0, W, W)
+            assert np.array_equal(gx, osx[M:M + W, M:M + W]), (wx0, wy0, o.counters()["mcs"])
+            assert np.array_equal(gy, osy[M:M + W, M:M + W]), (wx0, wy0, o.counters()["mcs"])
+            if wx0 + W > self.L and wy0 + W > self.L:       # the window holds site (0,0): its tracked height
+                assert k.counters()["h00"] == o.counters()["h00"]
+
+
+def _edge_windows(L, W):
+    """>= 8 windows: the corner that holds (0,0), the four lattice edges (each wrapping), and interior ones."""
+    h = W // 2
+    return [(L - h, L - h), (L - h, L // 3), (L // 5, L - h), (L - h, 7 * (L // 8)), (3 * (L // 4) + 11, L - h),
+            (50000 % L, 77777 % L), (L // 2 - 100, 3), (12345 % L, L // 2 + 4321)]
 
 
 def test_config3_full_size_windows_and_invariants(pkg):
     """BASELINE config 3 at full size (L=2^17, T=64, p=1, q=0, seed 42), in the launch configuration bench.py
-    times: sampled windows vs the light-cone window oracle + properties that hold at any size."""
+    times: eight 512^2 windows (the corner holding (0,0), all four lattice edges, interior) against the light-cone
+    window oracle at t = 1, 2, 4, 8, plus the properties that hold at any size."""
     import torch
     torch.cuda.empty_cache()
-    L, T, seed, n = 1 << 17, 64, 42, 4
+    L, T, seed = 1 << 17, 64, 42
     k = pkg.KPZ(L, 1.0, 0.0, T, seed)
     k.init_flat()
-    k.run(n)
     s1, s2, w2 = k.measure()
-    c = k.counters()
-    assert c["removals"] == 0 and c["attempts"] == n * L * L
-    assert int(s1[0]) - L * L // 2 == 2 * c["deposits"]            # +2 per accepted flip, exactly
-    assert 0.25 < w2[0] < 1.5
-    _window_check(pkg, k, L, T, 1.0, 0.0, seed, n, L - 300, L - 300, 600, check_h00=True)   # wraps, holds (0,0)
-    _window_check(pkg, k, L, T, 1.0, 0.0, seed, n, 50000, 77777, 512)
-    _window_check(pkg, k, L, T, 1.0, 0.0, seed, n, L // 2 - 100, 3, 512)
+    assert (int(s1[0]), int(s2[0]), float(w2[0])) == (L * L // 2, L * L // 2, 0.25)       # P:88, exact at full size
+    ws = _WindowSet(L, T, 1.0, 0.0, seed, 8, _edge_windows(L, 512), 512)
+    t = 0
+    for ts in (1, 2, 4, 8):
+        k.run(ts - t); ws.run(ts - t)
+        t = ts
+        ws.check(k)
+        s1, s2, w2 = k.measure()
+        c = k.counters()
+        assert c["removals"] == 0 and c["attempts"] == t * L * L and c["mcs"] == t
+        assert int(s1[0]) - L * L // 2 == 2 * c["deposits"]            # +2 per accepted flip, exactly
     k.close()
     torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("L", [1 << 17, 1 << 19])
+def test_flat_start_exact_sums_at_full_size(pkg, L):
+    """kpz_init_flat + kpz_measure at the sizes of configs 3 and 5: sum h = sum h^2 = L^2/2, W^2 = 1/4 -- the
+    exact pin of the measurement kernels (128 / 512 row chunks per column, word indices beyond 2^32 at 2^19) that
+    needs no host array."""
+    import torch
+    torch.cuda.empty_cache()
+    free_bytes, _ = torch.cuda.mem_get_info()
+    need = pkg.workspace_bytes(L, 64, 1)
+    if free_bytes < need[0] + need[1] + (2 << 30):
+        pytest.skip("SKIPPED: GPU has %.0f GiB free, L=%d needs %.0f GiB" % (free_bytes / 2**30, L, sum(need) / 2**30))
+    k = pkg.KPZ(L, 1.0, 0.0, 64, 1)
+    k.init_flat()
+    s1, s2, w2 = k.measure()
+    assert int(s1[0]) == L * L // 2 and int(s2[0]) == L * L // 2 and float(w2[0]) == 0.25
+    o = Oracle(L, 1.0, 0.0, 64, 1, window=(L - 64, L - 64, 128, 128))
+    o.init_flat()
+    gx, gy = k.get_window(L - 64, L - 64, 128, 128)
+    osx, osy = o.slopes()
+    assert np.array_equal(gx, osx) and np.array_equal(gy, osy)
+    k.close()
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("p,q,seed", [(1.0, 0.0, 42), (0.75, 0.25, 3)])
+def test_full_lattice_parity_2p16(pkg, p, q, seed):
+    """full parity at L = 2^16, T = 64 with the parameters of config 3 (p=1, q=0, seed 42) and of
+    config 5 (p=3/4, q=1/4, seed 3; option (i) of the config table): the FULL oracle (8 GiB of int8 slopes) for
+    3 MCS; state hash, sum h, sum h^2, W^2 and all counters after every MCS, and the full lattice at the end on
+    four quadrant-sized strips.  64 row chunks per column in the measurement kernels."""
+    import torch
+    L, T, n = 1 << 16, 64, 3
+    if _host_ram_gib() < 14:
+        print("SKIPPED test_full_lattice_parity_2p16: host RAM %.0f GiB < 14 GiB" % _host_ram_gib())
+        pytest.skip("host RAM")
+    torch.cuda.empty_cache()
+    k = pkg.KPZ(L, p, q, T, seed)
+    k.init_flat()
+    o = Oracle(L, p, q, T, seed, threads=NTHREADS)
+    o.init_flat()
+    for t in range(n):
+        k.run(1); o.run(1)
+        _compare_scalars(k, [o])
+        assert k.state_hash() == o.state_hash()
+    osx, osy = o.slopes()
+    for y0 in (0, L // 2 - 500, L - 1000):                   # full-width strips, element by element
+        gx, gy = k.get_window(0, y0, L, 1000)
+        assert np.array_equal(gx, osx[y0:y0 + 1000]) and np.array_equal(gy, osy[y0:y0 + 1000])
+    k.close()
+    torch.cuda.empty_cache()
+
+
+def test_config3_full_oracle_2p17(pkg):
+    """BASELINE config 3 itself against the FULL oracle (L = 2^17: 32 GiB of int8 slopes, about a minute per MCS on
+    16 cores): state hash, sum h, sum h^2, W^2, counters after MCS 1 and 2.  Skipped, loudly, only when the host has
+    less than 40 GiB of free RAM."""
+    import torch
+    L, T, seed, n = 1 << 17, 64, 42, 2
+    if _host_ram_gib() < 40 or os.environ.get("KPZ_TEST_FULL_2P17", "1") != "1":
+        print("SKIPPED test_config3_full_oracle_2p17: host RAM %.0f GiB < 40 GiB (or KPZ_TEST_FULL_2P17=0)" % _host_ram_gib())
+        pytest.skip("host RAM")
+    torch.cuda.empty_cache()
+    k = pkg.KPZ(L, 1.0, 0.0, T, seed)
+    k.init_flat()
+    o = Oracle(L, 1.0, 0.0, T, seed, threads=NTHREADS)
+    o.init_flat()
+    for t in range(n):
+        k.run(1); o.run(1)
+        _compare_scalars(k, [o])
+        assert k.state_hash() == o.state_hash()
+    k.close()
+    del o
+    torch.cuda.empty_cache()
+
+
+def test_blocked_lane_mapping_with_replicas(pkg):
+    """The 8x4 lane blocking of tiles (HN % 8 == 0) together with n_replicas > 1 -- the launch shape of the config-4
+    L = 2048 ensembles -- for T = 64 / general (p,q) and T = 16 / p = 1."""
+    for (L, T, p, q, R, n) in ((1024, 64, 0.75, 0.25, 3, 2), (256, 16, 1.0, 0.0, 5, 3)):
+        k = pkg.KPZ(L, p, q, T, 19, n_replicas=R)
+        k.init_flat()
+        os_ = [Oracle(L, p, q, T, 19, replica=r, threads=NTHREADS) for r in range(R)]
+        for o in os_:
+            o.init_flat()
+            o.run(n)
+        k.run(n)
+        _compare_scalars(k, os_)
+        for r in range(R):
+            _compare_full(k, os_[r], replica=r)
+            assert k.state_hash(r) == os_[r].state_hash()
+
+
+def test_mcs_clock_near_2p32(pkg):
+    """The MCS clock is Philox counter word c2 (S1): a trajectory started at clock 2^32 - 3 runs two
+    more MCS bit-exactly and refuses the next one (KPZ_EINVAL), on both sides."""
+    import torch
+    L, T, seed, start = 256, 16, 5, 2**32 - 3
+    k = pkg.KPZ(L, 0.75, 0.25, T, seed)
+    k.init_flat()
+    host = torch.empty(k.lattice_bytes, dtype=torch.uint8).pin_memory()
+    k.export_packed(host)
+    k.import_packed(host, np.zeros(1, dtype=np.int64), start)
+    o = Oracle(L, 0.75, 0.25, T, seed)
+    o.init_flat(); o.set_clock(start)
+    k.run(2); o.run(2)
+    _compare_full(k, o)
+    _compare_scalars(k, [o])
+    assert k.counters()["mcs"] == 2**32 - 1
+    with pytest.raises(pkg.KpzError) as e:
+        k.run(1)
+    assert e.value.code == pkg.KPZ_EINVAL
+    with pytest.raises(RuntimeError):
+        o.run(1)
+    assert k.state_hash() == o.state_hash()               # the refused call changed nothing
+    with pytest.raises(pkg.KpzError):
+        k.import_packed(host, np.zeros(1, dtype=np.int64), 2**32)
 
 
 def test_config5_shape_general_pq(pkg):
@@ -311,14 +464,18 @@ def test_config5_shape_general_pq(pkg):
     free_bytes, _ = torch.cuda.mem_get_info()
     if os.environ.get("KPZ_TEST_2P19", "1") == "1" and free_bytes > 72 * 2**30:
         torch.cuda.empty_cache()
-        L, n = 1 << 19, 2
+        L = 1 << 19
         k = pkg.KPZ(L, 0.75, 0.25, T, seed)
-        k.init_flat(); k.run(n)
-        s1, s2, w2 = k.measure()
-        c = k.counters()
-        assert int(s1[0]) - L * L // 2 == 2 * (c["deposits"] - c["removals"])
-        _window_check(pkg, k, L, T, 0.75, 0.25, seed, n, L - 256, L - 256, 512, check_h00=True)
-        _window_check(pkg, k, L, T, 0.75, 0.25, seed, n, 400000, 123456, 512)
+        k.init_flat()
+        ws = _WindowSet(L, T, 0.75, 0.25, seed, 4, _edge_windows(L, 512), 512)
+        t = 0
+        for ts in (1, 2, 4):
+            k.run(ts - t); ws.run(ts - t)
+            t = ts
+            ws.check(k)
+            s1, s2, w2 = k.measure()
+            c = k.counters()
+            assert int(s1[0]) - L * L // 2 == 2 * (c["deposits"] - c["removals"]) and c["attempts"] == t * L * L
         k.close()
         torch.cuda.empty_cache()
 

@@ -253,3 +253,33 @@ def test_mcs_is_exactly_L2_attempts_and_each_tile_gets_T2():
         if not order or order[-1] != col:
             order.append(col)
     assert order == perm
+
+
+def test_set_clock_restarts_a_trajectory_and_parallel_measure_is_thread_independent():
+    """set_clock only moves the MCS clock (S1: counter word c2): a lattice copied out after 2 MCS and
+    restarted at clock 2 continues the original trajectory bit for bit; the clock stops at 2^32 - 1.  The
+    measurement and the hash do not depend on the number of threads of their column / site loops."""
+    L, T, seed = 64, 16, 9
+    a = Oracle(L, 0.75, 0.25, T, seed)
+    a.init_flat(); a.run(2)
+    sx, sy = a.slopes()
+    h00 = a.counters()["h00"]
+    a.run(1)
+    b = Oracle(L, 0.75, 0.25, T, seed, threads=4)
+    b.set_slopes(sx, sy, h00=h00)
+    b.set_clock(2)
+    b.run(1)
+    bx, by = b.slopes()
+    ax, ay = a.slopes()
+    assert np.array_equal(ax, bx) and np.array_equal(ay, by)
+    assert a.measure() == b.measure() and a.state_hash() == b.state_hash()
+    assert b.counters()["mcs"] == 3 and b.counters()["attempts"] == 3 * L * L
+    h = gen.heights_to_slopes(ax.astype(np.int64).cumsum(axis=1) * 0 + Oracle.heights(a).astype(np.int64))
+    assert np.array_equal(h[0], ax) and np.array_equal(h[1], ay)        # heights() inverts to the same slopes
+    c = Oracle(L, 1.0, 0.0, T, seed)
+    c.init_flat(); c.set_clock(2**32 - 2)
+    c.run(1)
+    with pytest.raises(RuntimeError):
+        c.run(1)
+    with pytest.raises(ValueError):
+        c.set_clock(2**32)

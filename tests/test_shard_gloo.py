@@ -63,3 +63,26 @@ def test_single_process_defaults_and_slices():
         assert max(h - l for l, h in parts) - min(h - l for l, h in parts) <= 1
     with pytest.raises(ValueError):
         shard.replica_slice(4, 4, 4)
+
+
+def test_bench_gpus_2_starts_two_ranks_itself():
+    """`python bench.py --gpus 2` with no torchrun environment (the way the driver calls it for N = 1, and what a
+    user types for N > 1) must start the two ranks itself: the launcher self-test joins a gloo group of world size
+    2 through that path and reports n_gpus = 2; a WORLD_SIZE that contradicts --gpus is refused."""
+    import json
+    import subprocess
+    import sys
+    from pathlib import Path
+    root = Path(__file__).resolve().parent.parent
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, str(root / "bench.py"), "--gpus", "2", "--launcher-selftest"],
+                         capture_output=True, text=True, timeout=300, cwd=str(root), env=env)
+    assert out.returncode == 0, out.stderr[-800:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["units"] == 300.0 and d["seconds"] == 2.0 and d["seeds"] == [42, 43]
+    env["WORLD_SIZE"] = "1"
+    bad = subprocess.run([sys.executable, str(root / "bench.py"), "--gpus", "2", "--launcher-selftest"],
+                         capture_output=True, text=True, timeout=300, cwd=str(root), env=env)
+    assert bad.returncode != 0 and "WORLD_SIZE" in (bad.stderr + bad.stdout)
