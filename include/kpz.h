@@ -74,10 +74,26 @@ int32_t kpz_bind(kpz_ctx* ctx, void* d_lattice, size_t lattice_bytes, void* d_sc
  * W^2 = 1/4.  Resets h(0,0) = 0, the MCS clock and all counters of every replica.  Asynchronous. */
 int32_t kpz_init_flat(kpz_ctx* ctx);
 
-/* Advances every replica by `mcs` Monte Carlo steps (each exactly L*L attempts, 4 kernel launches).
+/* Advances every replica by `mcs` Monte Carlo steps (each exactly L*L attempts; 4 kernel launches per MCS on the
+ * tiled path, one launch per call on the lattice-resident path, see kpz_set_path).
  * Asynchronous on the bound stream.  kpz_run(a); kpz_run(b) == kpz_run(a+b).  KPZ_EINVAL if the MCS clock
  * would pass 2^32 - 1 (it is a 32-bit Philox counter word). */
 int32_t kpz_run(kpz_ctx* ctx, uint64_t mcs);
+
+/* Chooses the kernels kpz_run uses; the results are bit-identical on every path:
+ *   KPZ_PATH_AUTO (default): the lattice-resident kernels when L is a power of two <= 512, the schedule is the
+ *     default S4 without sub-sweeps or Poissonised counts and the height bits of a replica fit in shared memory
+ *     -- one warp per tile (warp-cooperative sequential updates) when the handle has at most 2048 tiles per colour
+ *     over all replicas, one thread per tile otherwise -- else the tiled kernel;
+ *   KPZ_PATH_TILED: kpz_update_kernel, one launch per colour pass (4 per MCS), any valid L;
+ *   KPZ_PATH_RESIDENT / KPZ_PATH_RESIDENT_COOP: force the one-thread-per-tile / one-warp-per-tile resident kernel
+ *     (one launch per kpz_run call); kpz_run then returns KPZ_EINVAL when the lattice or the schedule does not allow it.
+ * KPZ_EINVAL for any other value. */
+#define KPZ_PATH_AUTO 0
+#define KPZ_PATH_TILED 1
+#define KPZ_PATH_RESIDENT 2
+#define KPZ_PATH_RESIDENT_COOP 3
+int32_t kpz_set_path(kpz_ctx* ctx, int32_t path);
 
 /* Chooses the domain-decomposition schedule for subsequent kpz_run calls:
  *   KPZ_SCHEDULE_COLOURS (default): S4 -- four tile colours in random order, halo write-back, exactly L*L effective

@@ -22,6 +22,7 @@ exported_symbols = [
     "kpz_destroy", "kpz_synchronize", "kpz_last_error", "kpz_get_slopes", "kpz_get_window", "kpz_set_slopes",
     "kpz_state_hash", "kpz_counters", "kpz_export_packed", "kpz_import_packed", "kpz_step_host", "kpz_pipeline_host",
     "kpz_launch_count", "kpz_philox_selftest", "kpz_profiles", "kpz_power_spectrum", "kpz_set_schedule", "kpz_set_sub_sweeps", "kpz_run_sampled", "kpz_set_poisson",
+    "kpz_set_path",
 ]
 
 
@@ -60,6 +61,7 @@ def load_library() -> ctypes.CDLL:
         "kpz_run_sampled": [vp, vp, u32, vp, vp, vp],
         "kpz_set_schedule": [vp, i32],
         "kpz_set_poisson": [vp, i32],
+        "kpz_set_path": [vp, i32],
         "kpz_set_sub_sweeps": [vp, u32],
         "kpz_profiles": [vp, u32, vp, vp],
         "kpz_power_spectrum": [vp, u32, vp, vp, vp],
@@ -184,6 +186,11 @@ class KPZ:
     def set_schedule(self, name):
         """kpz_set_schedule: 'colours' (default) or 'dead_border' (the paper's own scheme)."""
         self._check(self._lib.kpz_set_schedule(self._h, {"colours": 0, "dead_border": 1}[name]))
+
+    def set_path(self, name):
+        """kpz_set_path: 'auto' (default), 'tiled', 'resident' (one thread per tile) or 'resident_coop' (one warp per
+        tile); the results are bit-identical."""
+        self._check(self._lib.kpz_set_path(self._h, {"auto": 0, "tiled": 1, "resident": 2, "resident_coop": 3}[name]))
 
     def set_poisson(self, on=True):
         """kpz_set_poisson: Poissonised number of steps per tile and sub-sweep (S7)."""

@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "kpz_device.cuh"
+#include "kpz_resident.cuh"
 
 namespace {
 
@@ -95,6 +96,7 @@ struct kpz_ctx {
     int32_t schedule;        // KPZ_SCHEDULE_COLOURS or KPZ_SCHEDULE_DEAD_BORDER
     uint32_t sub_sweeps;     // K sub-sweeps per MCS (S6)
     bool poisson;            // Poissonised steps per tile and sub-sweep (S7)
+    int32_t path;            // KPZ_PATH_*: which update kernels kpz_run uses
     uint32_t pn, pk_min;     // count table on the device (scratch ptab): entries, smallest count
     uint64_t attempts_base;  // attempts made by fixed-count MCS (S7 MCS count theirs on the device, stats[3])
     uint32_t* d_lattice;
@@ -225,6 +227,105 @@ int32_t launch_update(kpz_ctx* c, uint32_t m, uint32_t slot, uint32_t sub) {
     return fail(c, KPZ_EINVAL, "unsupported tile %u", c->T);
 }
 
+// ---- lattice-resident path (kpz_resident.cuh): one launch for all `n` MCS ------------------------------------
+struct ResidentPlan {
+    bool ok;            // the lattice fits and the schedule is the default one
+    bool coop;          // one warp per tile (few tiles) instead of one thread per tile
+    uint32_t G, threads, blocks;
+    size_t smem;
+};
+
+constexpr size_t KPZ_RESIDENT_SMEM_MAX = 200 * 1024;
+
+ResidentPlan resident_plan(const kpz_ctx* c, bool coop) {
+    ResidentPlan pl{};
+    const uint32_t L = c->L, T = c->T;
+    const bool general = !(c->p >= 1.0 && c->q <= 0.0);
+    const size_t lat = (size_t)L * L / 8;                    // bytes of height bits per replica
+    const uint32_t HN = L / T / 2, tpc = HN * HN;
+    pl.coop = coop;
+    pl.ok = (L & (L - 1)) == 0 && c->schedule == KPZ_SCHEDULE_COLOURS && c->sub_sweeps == 1 && !c->poisson;
+    if (!pl.ok) return pl;
+    if (coop) {
+        const uint32_t nwarps = tpc < 32u ? tpc : 32u;
+        pl.G = 1;
+        pl.threads = 32u * nwarps;
+        pl.blocks = c->R;
+        pl.smem = (general ? 3 : 2) * lat + (size_t)nwarps * kpz::KPZ_COOP_WARP_WORDS * 4;
+    } else {
+        uint32_t G = tpc >= 32u ? 1u : (32u + tpc - 1u) / tpc;     // fill at least one warp
+        if (G > c->R) G = c->R;
+        while (G > 1 && G * lat > KPZ_RESIDENT_SMEM_MAX) --G;
+        const uint64_t items = (uint64_t)G * tpc;
+        pl.G = G;
+        pl.threads = (uint32_t)(items > 1024 ? 1024 : (items + 31) / 32 * 32);
+        pl.blocks = (c->R + G - 1) / G;
+        pl.smem = G * lat;
+    }
+    pl.ok = pl.smem <= KPZ_RESIDENT_SMEM_MAX;
+    return pl;
+}
+
+template <int T, bool GENERAL, bool COOP>
+int32_t launch_resident_k(kpz_ctx* c, const kpz::ResidentParams& P, const ResidentPlan& pl) {
+    auto kern = kpz::kpz_resident_kernel<T, GENERAL, COOP>;
+    static bool attr_set[KPZ_MAX_DEVICES] = {};
+    const int dev = (c->device >= 0 && c->device < KPZ_MAX_DEVICES) ? c->device : 0;
+    if (!attr_set[dev]) {
+        KPZ_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)KPZ_RESIDENT_SMEM_MAX));
+        attr_set[dev] = true;
+    }
+    kern<<<pl.blocks, pl.threads, pl.smem, c->stream>>>(P);
+    KPZ_CUDA(c, cudaGetLastError());
+    c->launches++;
+    return KPZ_OK;
+}
+
+template <int T>
+int32_t launch_resident_t(kpz_ctx* c, const kpz::ResidentParams& P, const ResidentPlan& pl) {
+    const bool general = !(c->p >= 1.0 && c->q <= 0.0);
+    if (pl.coop) return general ? launch_resident_k<T, true, true>(c, P, pl) : launch_resident_k<T, false, true>(c, P, pl);
+    return general ? launch_resident_k<T, true, false>(c, P, pl) : launch_resident_k<T, false, false>(c, P, pl);
+}
+
+int32_t launch_resident(kpz_ctx* c, const ResidentPlan& pl, uint32_t m0, uint32_t n_mcs) {
+    kpz::ResidentParams P;
+    P.lattice = c->d_lattice;
+    P.stats = reinterpret_cast<unsigned long long*>(c->d_scratch + c->sl.stats);
+    P.plane_words = (uint64_t)c->L * c->L / 32;
+    P.thr_p = accept_threshold(c->p);
+    P.thr_q = accept_threshold(c->q);
+    P.L = c->L; P.W = c->L / 32; P.NT = c->L / c->T; P.HN = P.NT / 2; P.tpc = P.HN * P.HN;
+    P.R = c->R; P.G = pl.G; P.m0 = m0; P.n_mcs = n_mcs;
+    P.key.k0 = (uint32_t)(c->seed & 0xFFFFFFFFull);
+    P.key.k1 = (uint32_t)(c->seed >> 32);
+    switch (c->T) {
+        case 64: return launch_resident_t<64>(c, P, pl);
+        case 32: return launch_resident_t<32>(c, P, pl);
+        case 16: return launch_resident_t<16>(c, P, pl);
+        case 8: return launch_resident_t<8>(c, P, pl);
+        case 4: return launch_resident_t<4>(c, P, pl);
+    }
+    return fail(c, KPZ_EINVAL, "unsupported tile %u", c->T);
+}
+
+// Which kernels advance the lattice.  AUTO: the resident kernels when the lattice fits in shared memory and at most
+// L = 512 -- one warp per tile when the whole handle has few tiles per colour (a chain-bound lattice), one thread
+// per tile otherwise -- else the tiled kernel.
+int32_t choose_path(kpz_ctx* c, ResidentPlan& pl) {
+    const uint64_t tpc = (uint64_t)(c->L / c->T / 2) * (c->L / c->T / 2);
+    if (c->path == KPZ_PATH_TILED) return KPZ_PATH_TILED;
+    if (c->path == KPZ_PATH_RESIDENT || c->path == KPZ_PATH_RESIDENT_COOP) {
+        pl = resident_plan(c, c->path == KPZ_PATH_RESIDENT_COOP);
+        return pl.ok ? c->path : -1;
+    }
+    if (c->L > 512) return KPZ_PATH_TILED;
+    const bool coop = (uint64_t)c->R * tpc <= 2048;
+    pl = resident_plan(c, coop);
+    if (pl.ok) return coop ? KPZ_PATH_RESIDENT_COOP : KPZ_PATH_RESIDENT;
+    return KPZ_PATH_TILED;
+}
+
 int32_t require_bound(kpz_ctx* c) {
     if (!c) return KPZ_EINVAL;
     if (!c->bound) return fail(c, KPZ_ESTATE, "kpz_bind has not been called");
@@ -297,7 +398,7 @@ int32_t kpz_create_batch(kpz_ctx** out, uint32_t L, double p, double q, uint32_t
     if (!c) return KPZ_ENOMEM;
     c->L = L; c->T = tile; c->R = n_replicas; c->p = p; c->q = q; c->seed = seed;
     c->mcs = 0; c->launches = 0; c->schedule = KPZ_SCHEDULE_COLOURS; c->sub_sweeps = 1;
-    c->poisson = false; c->pn = 0; c->pk_min = 0; c->attempts_base = 0;
+    c->poisson = false; c->pn = 0; c->pk_min = 0; c->attempts_base = 0; c->path = KPZ_PATH_AUTO;
     c->d_lattice = nullptr; c->d_scratch = nullptr; c->stream = nullptr; c->bound = false; c->device = -1;
     c->sl = scratch_layout(L, n_replicas);
     c->lattice_bytes = (size_t)n_replicas * ((size_t)L * L / 4);
@@ -353,6 +454,17 @@ int32_t kpz_run(kpz_ctx* c, uint64_t mcs) {
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
     if (c->mcs + mcs > 0xFFFFFFFFull) return fail(c, KPZ_EINVAL, "MCS clock would exceed 2^32-1");
+    if (mcs == 0) return KPZ_OK;
+    ResidentPlan pl{};
+    const int32_t path = choose_path(c, pl);
+    if (path < 0) return fail(c, KPZ_EINVAL, "the resident path needs a power-of-two L that fits in shared memory and the default schedule");
+    if (path != KPZ_PATH_TILED) {
+        rc = launch_resident(c, pl, (uint32_t)c->mcs, (uint32_t)mcs);
+        if (rc != KPZ_OK) return rc;
+        c->mcs += mcs;
+        c->attempts_base += mcs * (uint64_t)c->L * c->L;
+        return KPZ_OK;
+    }
     for (uint64_t k = 0; k < mcs; ++k) {
         const uint32_t m = (uint32_t)c->mcs;
         const uint32_t passes = (c->schedule == KPZ_SCHEDULE_DEAD_BORDER) ? 1u : 4u;
@@ -365,6 +477,13 @@ int32_t kpz_run(kpz_ctx* c, uint64_t mcs) {
         c->mcs++;
         if (!c->poisson) c->attempts_base += (uint64_t)c->L * c->L;
     }
+    return KPZ_OK;
+}
+
+int32_t kpz_set_path(kpz_ctx* c, int32_t path) {
+    if (!c) return KPZ_EINVAL;
+    if (path < KPZ_PATH_AUTO || path > KPZ_PATH_RESIDENT_COOP) return fail(c, KPZ_EINVAL, "unknown path");
+    c->path = path;
     return KPZ_OK;
 }
 

@@ -153,7 +153,9 @@ def _compare_scalars(k, os_, replica_slice=None):
     (128, 32, 1.0, 0.4, 15, 3),        # p = 1 with removals: inclusive 32-bit threshold 2^32 - 1
 ])
 def test_update_parity_every_mcs(pkg, L, T, p, q, seed, n):
+    """The tiled kernel (kpz_update_kernel, forced: small lattices would otherwise take the resident path)."""
     k = pkg.KPZ(L, p, q, T, seed)
+    k.set_path("tiled")
     k.init_flat()
     o = Oracle(L, p, q, T, seed, threads=NTHREADS)
     o.init_flat()
@@ -163,6 +165,78 @@ def test_update_parity_every_mcs(pkg, L, T, p, q, seed, n):
         _compare_full(k, o)
         _compare_scalars(k, [o])
         assert k.state_hash() == o.state_hash()
+
+
+@pytest.mark.parametrize("path", ["resident", "resident_coop", "auto"])
+@pytest.mark.parametrize("L,T,p,q,seed,R,n", [
+    (32, 4, 1.0, 0.0, 61, 1, 5),           # one word per row, 16 steps per tile: half a warp batch
+    (32, 4, 0.75, 0.25, 62, 7, 4),
+    (64, 8, 0.75, 0.25, 63, 3, 4),
+    (64, 16, 0.5, 0.0, 64, 2, 4),          # a probability of exactly 0
+    (128, 16, 1.0, 0.0, 4, 6, 5),          # config-4 shape
+    (128, 32, 0.3, 0.9, 65, 1, 4),
+    (128, 64, 0.0, 0.7, 66, 2, 3),         # a single tile per colour
+    (256, 16, 1.0, 0.0, 1, 1, 6),          # config 1
+    (256, 64, 0.75, 0.25, 3, 1, 3),
+    (512, 16, 1.0, 0.0, 67, 1, 2),
+    (512, 32, 0.6, 0.1, 68, 2, 2),
+])
+def test_resident_paths_parity(pkg, path, L, T, p, q, seed, R, n):
+    """Lattice-resident kernels (kpz_resident_kernel: one thread per tile / one warp per tile, whole lattice in shared
+    memory, n MCS per launch): state, sums, counters after every MCS, then n more MCS in ONE launch."""
+    k = pkg.KPZ(L, p, q, T, seed, n_replicas=R)
+    k.set_path(path)
+    k.init_flat()
+    os_ = [Oracle(L, p, q, T, seed, replica=r, threads=NTHREADS) for r in range(R)]
+    for o in os_:
+        o.init_flat()
+    for t in range(n):
+        l0 = k.launch_count()
+        k.run(1)
+        assert k.launch_count() - l0 == 1          # one launch per call, not four per MCS
+        for o in os_:
+            o.run(1)
+        _compare_scalars(k, os_)
+        for r in range(R):
+            _compare_full(k, os_[r], replica=r)
+    l0 = k.launch_count()
+    k.run(n)
+    assert k.launch_count() - l0 == 1
+    for o in os_:
+        o.run(n)
+    _compare_scalars(k, os_)
+    for r in range(R):
+        assert k.state_hash(r) == os_[r].state_hash()
+    # switching to the tiled kernel mid-run continues the same trajectory
+    k.set_path("tiled")
+    k.run(1)
+    for o in os_:
+        o.run(1)
+    _compare_scalars(k, os_)
+    _compare_full(k, os_[R - 1], replica=R - 1)
+
+
+def test_resident_path_is_refused_when_it_cannot_hold_the_lattice(pkg):
+    for (L, T, path) in ((96, 16, "resident"), (2048, 16, "resident"), (1024, 64, "resident_coop")):
+        k = pkg.KPZ(L, 1.0, 0.0, T, 1)
+        k.set_path(path)
+        k.init_flat()
+        with pytest.raises(pkg.KpzError) as e:
+            k.run(1)
+        assert e.value.code == pkg.KPZ_EINVAL
+        k.set_path("auto")
+        k.run(1)
+        o = Oracle(L, 1.0, 0.0, T, 1, threads=NTHREADS)
+        o.init_flat(); o.run(1)
+        assert k.state_hash() == o.state_hash()
+    k = pkg.KPZ(128, 1.0, 0.0, 16, 1)
+    k.set_path("resident")
+    k.set_sub_sweeps(2)
+    k.init_flat()
+    with pytest.raises(pkg.KpzError):
+        k.run(1)                                   # sub-sweeps run on the tiled kernel only
+    with pytest.raises(KeyError):
+        k.set_path("nonsense")
 
 
 def test_config1_full(pkg):
