@@ -81,18 +81,17 @@ int32_t kpz_init_flat(kpz_ctx* ctx);
 int32_t kpz_run(kpz_ctx* ctx, uint64_t mcs);
 
 /* Chooses the kernels kpz_run uses; the results are bit-identical on every path:
- *   KPZ_PATH_AUTO (default): the lattice-resident kernels when L is a power of two <= 512, the schedule is the
- *     default S4 without sub-sweeps or Poissonised counts and the height bits of a replica fit in shared memory
- *     -- one warp per tile (warp-cooperative sequential updates) when the handle has at most 2048 tiles per colour
- *     over all replicas, one thread per tile otherwise -- else the tiled kernel;
+ *   KPZ_PATH_AUTO (default): the lattice-resident kernel when the packed lattice fits in shared memory (L <= 512),
+ *     the schedule is the default S4 without sub-sweeps or Poissonised counts and the handle is small enough to
+ *     be bound by launches and tile staging; else the tiled kernel;
  *   KPZ_PATH_TILED: kpz_update_kernel, one launch per colour pass (4 per MCS), any valid L;
- *   KPZ_PATH_RESIDENT / KPZ_PATH_RESIDENT_COOP: force the one-thread-per-tile / one-warp-per-tile resident kernel
- *     (one launch per kpz_run call); kpz_run then returns KPZ_EINVAL when the lattice or the schedule does not allow it.
+ *   KPZ_PATH_RESIDENT: force the resident kernel (one launch per kpz_run call, the lattices of a CTA's replicas
+ *     stay in shared memory for all MCS of the call); kpz_run then returns KPZ_EINVAL when the lattice or the
+ *     schedule does not allow it.
  * KPZ_EINVAL for any other value. */
 #define KPZ_PATH_AUTO 0
 #define KPZ_PATH_TILED 1
 #define KPZ_PATH_RESIDENT 2
-#define KPZ_PATH_RESIDENT_COOP 3
 int32_t kpz_set_path(kpz_ctx* ctx, int32_t path);
 
 /* Chooses the domain-decomposition schedule for subsequent kpz_run calls:
@@ -216,6 +215,20 @@ int32_t kpz_power_spectrum(kpz_ctx* ctx, uint32_t replica, double* S, double* Sx
 
 /* Number of kernels this handle has launched since creation (for bench.py "gpu_launches"). */
 int32_t kpz_launch_count(const kpz_ctx* ctx, uint64_t* out);
+
+/* Pipe micro-benchmarks for the roofline of the update kernel (MEASURED_PEAKS.json has no
+ * integer or shared-memory peak).  Runs, on the CURRENT device, kernels that only issue one kind of instruction from
+ * every warp slot of every SM and writes KPZ_N_PEAKS doubles to the HOST array `out` (n >= KPZ_N_PEAKS):
+ *   [0] SM clock in Hz during the run (clock64 ticks / CUDA-event time)
+ *   [1] LOP3, [2] SHF, [3] IMAD, [4] IMAD.WIDE throughput in lane-operations/s (32 per warp instruction)
+ *   [5] shared-memory LDS.32 bytes/s with every lane in its own bank (the tile layout of the update kernel)
+ *   [6] shared-memory XOR reductions (ATOMS / RED) in lane-operations/s
+ *   [7] attempts/s of the bare instruction mix of one p = 1, q = 0 attempt (5 LDS, 2 SHF, 3 LOP3, 1 reduction) issued
+ *       without the dependent chain of a real tile -- what the update kernel would reach with perfect latency hiding
+ *   [8] number of SMs.
+ * Takes a few tens of milliseconds.  KPZ_EINVAL for a NULL / short array, KPZ_ECUDA without a device. */
+#define KPZ_N_PEAKS 9
+int32_t kpz_measure_peaks(double* out, uint32_t n);
 
 /* Device Philox4x32-10 self-test: evaluates n (counter,key) inputs on the GPU.  HOST arrays: ctr[4n], key[2n],
  * out[4n].  Used by the tests to check the in-kernel generator against the published known answers. */

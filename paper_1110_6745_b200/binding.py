@@ -22,7 +22,7 @@ exported_symbols = [
     "kpz_destroy", "kpz_synchronize", "kpz_last_error", "kpz_get_slopes", "kpz_get_window", "kpz_set_slopes",
     "kpz_state_hash", "kpz_counters", "kpz_export_packed", "kpz_import_packed", "kpz_step_host", "kpz_pipeline_host",
     "kpz_launch_count", "kpz_philox_selftest", "kpz_profiles", "kpz_power_spectrum", "kpz_set_schedule", "kpz_set_sub_sweeps", "kpz_run_sampled", "kpz_set_poisson",
-    "kpz_set_path",
+    "kpz_set_path", "kpz_measure_peaks",
 ]
 
 
@@ -71,6 +71,7 @@ def load_library() -> ctypes.CDLL:
         "kpz_pipeline_host": [vp, vp, sz, u32, vp, sz, vp, vp, u64, u32, vp, vp, vp],
         "kpz_launch_count": [vp, vp],
         "kpz_philox_selftest": [vp, vp, vp, u32],
+        "kpz_measure_peaks": [vp, u32],
     }
     for name, args in sig.items():
         fn = getattr(L, name)
@@ -88,6 +89,19 @@ def workspace_bytes(L, tile, n_replicas=1):
     if rc != KPZ_OK:
         raise KpzError(rc)
     return a.value, b.value
+
+
+PEAK_NAMES = ("sm_clock_hz", "lop3_lane_ops", "shf_lane_ops", "imad_lane_ops", "imad_wide_lane_ops", "lds_bytes",
+              "smem_xor_lane_ops", "attempt_mix", "n_sms")
+
+
+def measure_peaks():
+    """kpz_measure_peaks on the current device -> dict of the nine figures (per second, see include/kpz.h)."""
+    out = np.zeros(len(PEAK_NAMES), dtype=np.float64)
+    rc = load_library().kpz_measure_peaks(out.ctypes.data, len(out))
+    if rc != KPZ_OK:
+        raise KpzError(rc, "kpz_measure_peaks")
+    return dict(zip(PEAK_NAMES, out.tolist()))
 
 
 def philox_selftest(ctr, key):
@@ -188,9 +202,9 @@ class KPZ:
         self._check(self._lib.kpz_set_schedule(self._h, {"colours": 0, "dead_border": 1}[name]))
 
     def set_path(self, name):
-        """kpz_set_path: 'auto' (default), 'tiled', 'resident' (one thread per tile) or 'resident_coop' (one warp per
-        tile); the results are bit-identical."""
-        self._check(self._lib.kpz_set_path(self._h, {"auto": 0, "tiled": 1, "resident": 2, "resident_coop": 3}[name]))
+        """kpz_set_path: 'auto' (default), 'tiled' or 'resident' (lattice kept in shared memory, one launch per run
+        call); the results are bit-identical."""
+        self._check(self._lib.kpz_set_path(self._h, {"auto": 0, "tiled": 1, "resident": 2}[name]))
 
     def set_poisson(self, on=True):
         """kpz_set_poisson: Poissonised number of steps per tile and sub-sweep (S7)."""

@@ -1,42 +1,19 @@
 // kpz.cu -- host side of libkpz_b200.so: the C ABI of include/kpz.h on top of the kernels in kpz_device.cuh.
 // No CPU fallback: every entry point that computes launches CUDA kernels on the bound stream.
-#include "../../include/kpz.h"
-
-#include <cuda_runtime.h>
+#include "kpz_host.h"
 
 #include <cmath>
-#include <cstdarg>
-#include <cstdio>
 #include <cstring>
 #include <new>
 #include <vector>
 
-#include "kpz_device.cuh"
-#include "kpz_resident.cuh"
+#include "kpz_aux_kernels.cuh"
+#include "kpz_peaks.cuh"
 
 namespace {
 
 typedef __int128 i128;
 typedef unsigned __int128 u128;
-
-struct ScratchLayout {
-    size_t stats;     // [R][4] u64 : deposits, removals, h00, reserved
-    size_t msum;      // [R][4] u64 : lo/hi halves of sum rel, sum rel^2
-    size_t misc;      // 8 x u64    : [0] hash accumulator, [1] validation flags
-    size_t base;      // [R][L] i32
-    size_t cS0;       // [R][NC][L] i32
-    size_t cS1;       // [R][NC][L] i32
-    size_t cS2;       // [R][NC][L] i32
-    size_t colsum;    // [L] i64       column sums of one replica (power spectrum / profiles)
-    size_t rowinc;    // [L] i32
-    size_t prof;      // [2][L] i64    column and row profiles relative to h00
-    size_t fft;       // [2][L] double2
-    size_t sdir;      // [2][L/2+1] double
-    size_t savg;      // [L/2+1] double
-    size_t ptab;      // [4096] u64     S7 count table
-    size_t total;
-    uint32_t n_chunks, rows_per_chunk;
-};
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -87,46 +64,7 @@ uint64_t accept_threshold(double prob) {
 
 }  // namespace
 
-struct kpz_ctx {
-    uint32_t L, T, R;
-    double p, q;
-    uint64_t seed;
-    uint64_t mcs;            // completed MCS (all replicas advance together)
-    uint64_t launches;
-    int32_t schedule;        // KPZ_SCHEDULE_COLOURS or KPZ_SCHEDULE_DEAD_BORDER
-    uint32_t sub_sweeps;     // K sub-sweeps per MCS (S6)
-    bool poisson;            // Poissonised steps per tile and sub-sweep (S7)
-    int32_t path;            // KPZ_PATH_*: which update kernels kpz_run uses
-    uint32_t pn, pk_min;     // count table on the device (scratch ptab): entries, smallest count
-    uint64_t attempts_base;  // attempts made by fixed-count MCS (S7 MCS count theirs on the device, stats[3])
-    uint32_t* d_lattice;
-    unsigned char* d_scratch;
-    cudaStream_t stream;
-    bool bound;
-    ScratchLayout sl;
-    size_t lattice_bytes;
-    int device;              // ordinal of the device that holds the bound buffers (-1 before kpz_bind)
-    char err[512];
-};
-
 namespace {
-
-int32_t fail(kpz_ctx* c, int32_t code, const char* fmt, ...) {
-    if (c) {
-        va_list ap;
-        va_start(ap, fmt);
-        vsnprintf(c->err, sizeof(c->err), fmt, ap);
-        va_end(ap);
-    }
-    return code;
-}
-
-#define KPZ_CUDA(c, expr)                                                                          \
-    do {                                                                                           \
-        cudaError_t e__ = (expr);                                                                  \
-        if (e__ != cudaSuccess)                                                                    \
-            return fail((c), KPZ_ECUDA, "%s failed: %s", #expr, cudaGetErrorString(e__));          \
-    } while (0)
 
 // Makes the handle's device current for the duration of an entry point and restores the caller's device.
 struct DeviceGuard {
@@ -142,7 +80,8 @@ struct DeviceGuard {
     DeviceGuard& operator=(const DeviceGuard&) = delete;
 };
 
-constexpr int KPZ_MAX_DEVICES = 64;
+// AUTO takes the resident path up to this many tiles per colour over all replicas (measured cross-over)
+constexpr uint64_t KPZ_RESIDENT_AUTO_MAX_TILES = 1u << 20;
 
 int grid_for(uint64_t n, int block, int cap = 148 * 16) {
     uint64_t g = (n + block - 1) / block;
@@ -151,47 +90,7 @@ int grid_for(uint64_t n, int block, int cap = 148 * 16) {
     return (int)g;
 }
 
-template <int T, int NTHR, int MODE, bool DEAD, int SUB>
-int32_t launch_update_k(kpz_ctx* c, const kpz::UpdateParams& P) {
-    const size_t smem = (size_t)kpz::TileGeom<T>::WORDS * NTHR * sizeof(uint32_t);
-    auto kern = kpz::kpz_update_kernel<T, NTHR, MODE, DEAD, SUB>;
-    // function attributes are per device: one flag per device ordinal and instantiation
-    static bool attr_set[KPZ_MAX_DEVICES] = {};
-    const int dev = (c->device >= 0 && c->device < KPZ_MAX_DEVICES) ? c->device : 0;
-    if (!attr_set[dev]) {
-        KPZ_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        KPZ_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-        attr_set[dev] = true;
-    }
-    const uint64_t blocks = (P.total_items + NTHR - 1) / NTHR;
-    if (blocks > 0x7FFFFFFFull) return fail(c, KPZ_EINVAL, "too many tiles for one launch");
-    kern<<<(unsigned)blocks, NTHR, smem, c->stream>>>(P);
-    KPZ_CUDA(c, cudaGetLastError());
-    c->launches++;
-    return KPZ_OK;
-}
-
-template <int T, int NTHR, int MODE, bool DEAD>
-int32_t launch_update_t(kpz_ctx* c, const kpz::UpdateParams& P) {
-    if (c->poisson) return launch_update_k<T, NTHR, MODE, DEAD, 2>(c, P);
-    return c->sub_sweeps > 1 ? launch_update_k<T, NTHR, MODE, DEAD, 1>(c, P) : launch_update_k<T, NTHR, MODE, DEAD, 0>(c, P);
-}
-
-template <int T, int NTHR, bool DEAD>
-int32_t launch_update_sched(kpz_ctx* c, const kpz::UpdateParams& P) {
-    if (c->p >= 1.0 && c->q <= 0.0) return launch_update_t<T, NTHR, 0, DEAD>(c, P);
-    if (P.thr_p >= 1 && P.thr_q >= 1) return launch_update_t<T, NTHR, 1, DEAD>(c, P);
-    return launch_update_t<T, NTHR, 2, DEAD>(c, P);
-}
-
-template <int T, int NTHR>
-int32_t launch_update_mode(kpz_ctx* c, const kpz::UpdateParams& P) {
-    return c->schedule == KPZ_SCHEDULE_DEAD_BORDER ? launch_update_sched<T, NTHR, true>(c, P)
-                                                   : launch_update_sched<T, NTHR, false>(c, P);
-}
-
-int32_t launch_update(kpz_ctx* c, uint32_t m, uint32_t slot, uint32_t sub) {
-    kpz::UpdateParams P;
+void fill_update_params(const kpz_ctx* c, kpz::UpdateParams& P, uint32_t m, uint32_t slot, uint32_t sub) {
     P.lattice = c->d_lattice;
     P.stats = reinterpret_cast<unsigned long long*>(c->d_scratch + c->sl.stats);
     P.plane_words = (uint64_t)c->L * c->L / 32;
@@ -217,118 +116,69 @@ int32_t launch_update(kpz_ctx* c, uint32_t m, uint32_t slot, uint32_t sub) {
     P.pk_min = c->pk_min;
     P.key.k0 = (uint32_t)(c->seed & 0xFFFFFFFFull);
     P.key.k1 = (uint32_t)(c->seed >> 32);
-    switch (c->T) {
-        case 64: return launch_update_mode<64, 96>(c, P);
-        case 32: return launch_update_mode<32, 64>(c, P);
-        case 16: return launch_update_mode<16, 128>(c, P);
-        case 8: return launch_update_mode<8, 128>(c, P);
-        case 4: return launch_update_mode<4, 128>(c, P);
-    }
-    return fail(c, KPZ_EINVAL, "unsupported tile %u", c->T);
 }
 
-// ---- lattice-resident path (kpz_resident.cuh): one launch for all `n` MCS ------------------------------------
-struct ResidentPlan {
-    bool ok;            // the lattice fits and the schedule is the default one
-    bool coop;          // one warp per tile (few tiles) instead of one thread per tile
-    uint32_t G, threads, blocks;
-    size_t smem;
-};
+int32_t launch_update(kpz_ctx* c, uint32_t m, uint32_t slot, uint32_t sub) {
+    kpz::UpdateParams P;
+    fill_update_params(c, P, m, slot, sub);
+    return c->T >= 32 ? kpz_launch_update_wide(c, P) : kpz_launch_update_narrow(c, P);
+}
 
-constexpr size_t KPZ_RESIDENT_SMEM_MAX = 200 * 1024;
+// ---- lattice-resident path (kpz_resident_kernel): one launch for all MCS of a kpz_run call -------------------
 
-ResidentPlan resident_plan(const kpz_ctx* c, bool coop) {
+size_t tile_words(uint32_t T) {
+    switch (T) {
+        case 64: return kpz::TileGeom<64>::WORDS;
+        case 32: return kpz::TileGeom<32>::WORDS;
+        case 16: return kpz::TileGeom<16>::WORDS;
+        case 8: return kpz::TileGeom<8>::WORDS;
+        default: return kpz::TileGeom<4>::WORDS;
+    }
+}
+
+ResidentPlan resident_plan(const kpz_ctx* c) {
     ResidentPlan pl{};
     const uint32_t L = c->L, T = c->T;
-    const bool general = !(c->p >= 1.0 && c->q <= 0.0);
-    const size_t lat = (size_t)L * L / 8;                    // bytes of height bits per replica
+    const size_t lat = (size_t)L * L / 4;                        // bytes of one packed lattice
     const uint32_t HN = L / T / 2, tpc = HN * HN;
-    pl.coop = coop;
-    pl.ok = (L & (L - 1)) == 0 && c->schedule == KPZ_SCHEDULE_COLOURS && c->sub_sweeps == 1 && !c->poisson;
+    pl.ok = c->schedule == KPZ_SCHEDULE_COLOURS && c->sub_sweeps == 1 && !c->poisson && lat <= KPZ_RESIDENT_SMEM_MAX;
     if (!pl.ok) return pl;
-    if (coop) {
-        const uint32_t nwarps = tpc < 32u ? tpc : 32u;
-        pl.G = 1;
-        pl.threads = 32u * nwarps;
-        pl.blocks = c->R;
-        pl.smem = (general ? 3 : 2) * lat + (size_t)nwarps * kpz::KPZ_COOP_WARP_WORDS * 4;
-    } else {
-        uint32_t G = tpc >= 32u ? 1u : (32u + tpc - 1u) / tpc;     // fill at least one warp
-        if (G > c->R) G = c->R;
-        while (G > 1 && G * lat > KPZ_RESIDENT_SMEM_MAX) --G;
-        const uint64_t items = (uint64_t)G * tpc;
-        pl.G = G;
-        pl.threads = (uint32_t)(items > 1024 ? 1024 : (items + 31) / 32 * 32);
-        pl.blocks = (c->R + G - 1) / G;
-        pl.smem = G * lat;
-    }
+    // threads per CTA: a multiple of 128 wherever the handle has the tiles for it.  Warps are bound to the four
+    // schedulers of an SM by their index inside the CTA, so single-warp CTAs would pile every chain of an SM onto
+    // one scheduler (measured: 1024 x L = 128 at 32 threads per CTA runs at half the rate of 128 threads per CTA).
+    const uint64_t all_tiles = (uint64_t)c->R * tpc;
+    pl.nthr = tpc >= 256u ? 256u : (all_tiles >= 128u ? 128u : (all_tiles >= 64u ? 64u : 32u));
+    uint32_t G = tpc >= pl.nthr ? 1u : pl.nthr / tpc;
+    if (G > c->R) G = c->R;
+    const size_t tiles = tile_words(T) * pl.nthr * 4;
+    while (G > 1 && G * lat + tiles > KPZ_RESIDENT_SMEM_MAX) --G;
+    pl.G = G;
+    pl.blocks = (c->R + G - 1) / G;
+    pl.smem = G * lat + tiles;
     pl.ok = pl.smem <= KPZ_RESIDENT_SMEM_MAX;
     return pl;
 }
 
-template <int T, bool GENERAL, bool COOP>
-int32_t launch_resident_k(kpz_ctx* c, const kpz::ResidentParams& P, const ResidentPlan& pl) {
-    auto kern = kpz::kpz_resident_kernel<T, GENERAL, COOP>;
-    static bool attr_set[KPZ_MAX_DEVICES] = {};
-    const int dev = (c->device >= 0 && c->device < KPZ_MAX_DEVICES) ? c->device : 0;
-    if (!attr_set[dev]) {
-        KPZ_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)KPZ_RESIDENT_SMEM_MAX));
-        attr_set[dev] = true;
-    }
-    kern<<<pl.blocks, pl.threads, pl.smem, c->stream>>>(P);
-    KPZ_CUDA(c, cudaGetLastError());
-    c->launches++;
-    return KPZ_OK;
-}
-
-template <int T>
-int32_t launch_resident_t(kpz_ctx* c, const kpz::ResidentParams& P, const ResidentPlan& pl) {
-    const bool general = !(c->p >= 1.0 && c->q <= 0.0);
-    if (pl.coop) return general ? launch_resident_k<T, true, true>(c, P, pl) : launch_resident_k<T, false, true>(c, P, pl);
-    return general ? launch_resident_k<T, true, false>(c, P, pl) : launch_resident_k<T, false, false>(c, P, pl);
-}
-
 int32_t launch_resident(kpz_ctx* c, const ResidentPlan& pl, uint32_t m0, uint32_t n_mcs) {
-    kpz::ResidentParams P;
-    P.lattice = c->d_lattice;
-    P.stats = reinterpret_cast<unsigned long long*>(c->d_scratch + c->sl.stats);
-    P.plane_words = (uint64_t)c->L * c->L / 32;
-    P.thr_p = accept_threshold(c->p);
-    P.thr_q = accept_threshold(c->q);
-    P.L = c->L; P.W = c->L / 32; P.NT = c->L / c->T; P.HN = P.NT / 2; P.tpc = P.HN * P.HN;
-    P.R = c->R; P.G = pl.G; P.m0 = m0; P.n_mcs = n_mcs;
-    P.key.k0 = (uint32_t)(c->seed & 0xFFFFFFFFull);
-    P.key.k1 = (uint32_t)(c->seed >> 32);
-    switch (c->T) {
-        case 64: return launch_resident_t<64>(c, P, pl);
-        case 32: return launch_resident_t<32>(c, P, pl);
-        case 16: return launch_resident_t<16>(c, P, pl);
-        case 8: return launch_resident_t<8>(c, P, pl);
-        case 4: return launch_resident_t<4>(c, P, pl);
-    }
-    return fail(c, KPZ_EINVAL, "unsupported tile %u", c->T);
+    kpz::UpdateParams P;
+    fill_update_params(c, P, m0, 0u, 0u);
+    return c->T >= 32 ? kpz_launch_resident_wide(c, P, pl, n_mcs) : kpz_launch_resident_narrow(c, P, pl, n_mcs);
 }
 
-// Which kernels advance the lattice.  AUTO: the resident kernels when the lattice fits in shared memory and at most
-// L = 512 -- one warp per tile when the whole handle has few tiles per colour (a chain-bound lattice), one thread
-// per tile otherwise -- else the tiled kernel.
+// Which kernels advance the lattice.  AUTO: the resident kernel when the packed lattice fits in shared memory
+// (L <= 512 in practice) and a colour has too few tiles to fill the GPU, else the tiled kernel.
 int32_t choose_path(kpz_ctx* c, ResidentPlan& pl) {
-    const uint64_t tpc = (uint64_t)(c->L / c->T / 2) * (c->L / c->T / 2);
     if (c->path == KPZ_PATH_TILED) return KPZ_PATH_TILED;
-    if (c->path == KPZ_PATH_RESIDENT || c->path == KPZ_PATH_RESIDENT_COOP) {
-        pl = resident_plan(c, c->path == KPZ_PATH_RESIDENT_COOP);
-        return pl.ok ? c->path : -1;
-    }
-    if (c->L > 512) return KPZ_PATH_TILED;
-    const bool coop = (uint64_t)c->R * tpc <= 2048;
-    pl = resident_plan(c, coop);
-    if (pl.ok) return coop ? KPZ_PATH_RESIDENT_COOP : KPZ_PATH_RESIDENT;
-    return KPZ_PATH_TILED;
+    pl = resident_plan(c);
+    if (c->path == KPZ_PATH_RESIDENT) return pl.ok ? KPZ_PATH_RESIDENT : -1;
+    if (!pl.ok) return KPZ_PATH_TILED;
+    const uint64_t tpc = (uint64_t)(c->L / c->T / 2) * (c->L / c->T / 2);
+    return ((uint64_t)c->R * tpc <= KPZ_RESIDENT_AUTO_MAX_TILES) ? KPZ_PATH_RESIDENT : KPZ_PATH_TILED;
 }
 
 int32_t require_bound(kpz_ctx* c) {
     if (!c) return KPZ_EINVAL;
-    if (!c->bound) return fail(c, KPZ_ESTATE, "kpz_bind has not been called");
+    if (!c->bound) return kpz_fail(c, KPZ_ESTATE, "kpz_bind has not been called");
     return KPZ_OK;
 }
 
@@ -375,6 +225,35 @@ bool fits_i64(i128 v) { return v >= (i128)INT64_MIN && v <= (i128)INT64_MAX; }
 
 }  // namespace
 
+namespace {
+
+template <int KIND>
+cudaError_t run_peak(uint32_t blocks, uint32_t iters, uint32_t* sink, unsigned long long* ticks, float* ms) {
+    cudaEvent_t e0, e1;
+    cudaError_t e = cudaEventCreate(&e0);
+    if (e != cudaSuccess) return e;
+    e = cudaEventCreate(&e1);
+    if (e != cudaSuccess) { cudaEventDestroy(e0); return e; }
+    kpz::kpz_peak_kernel<KIND><<<blocks, 256>>>(iters / 8 + 1, 0x9E3779B9u, sink, ticks);      // warm-up
+    float best = 1e30f;
+    for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {
+        cudaEventRecord(e0);
+        kpz::kpz_peak_kernel<KIND><<<blocks, 256>>>(iters, 0x9E3779B9u + rep, sink, ticks);
+        cudaEventRecord(e1);
+        e = cudaEventSynchronize(e1);
+        float t = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&t, e0, e1);
+        if (e == cudaSuccess && t < best) best = t;
+    }
+    if (e == cudaSuccess) e = cudaGetLastError();
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    *ms = best;
+    return e;
+}
+
+}  // namespace
+
 extern "C" {
 
 int32_t kpz_workspace_bytes(uint32_t L, uint32_t tile, uint32_t n_replicas, size_t* lattice_bytes,
@@ -399,7 +278,7 @@ int32_t kpz_create_batch(kpz_ctx** out, uint32_t L, double p, double q, uint32_t
     c->L = L; c->T = tile; c->R = n_replicas; c->p = p; c->q = q; c->seed = seed;
     c->mcs = 0; c->launches = 0; c->schedule = KPZ_SCHEDULE_COLOURS; c->sub_sweeps = 1;
     c->poisson = false; c->pn = 0; c->pk_min = 0; c->attempts_base = 0; c->path = KPZ_PATH_AUTO;
-    c->d_lattice = nullptr; c->d_scratch = nullptr; c->stream = nullptr; c->bound = false; c->device = -1;
+    c->d_lattice = nullptr; c->d_scratch = nullptr; c->stream = nullptr; c->bound = false; c->device = -1; c->s_in = nullptr; c->s_out = nullptr;
     c->sl = scratch_layout(L, n_replicas);
     c->lattice_bytes = (size_t)n_replicas * ((size_t)L * L / 4);
     c->err[0] = 0;
@@ -414,17 +293,17 @@ int32_t kpz_create(kpz_ctx** out, uint32_t L, double p, double q, uint32_t tile,
 int32_t kpz_bind(kpz_ctx* c, void* d_lattice, size_t lattice_bytes, void* d_scratch, size_t scratch_bytes,
                  void* cuda_stream) {
     if (!c) return KPZ_EINVAL;
-    if (!d_lattice || !d_scratch) return fail(c, KPZ_EINVAL, "NULL device buffer");
+    if (!d_lattice || !d_scratch) return kpz_fail(c, KPZ_EINVAL, "NULL device buffer");
     if (lattice_bytes < c->lattice_bytes || scratch_bytes < c->sl.total)
-        return fail(c, KPZ_ENOMEM, "bound buffers too small: need %zu + %zu bytes", c->lattice_bytes, c->sl.total);
-    if (((uintptr_t)d_lattice & 15u) || ((uintptr_t)d_scratch & 15u)) return fail(c, KPZ_EINVAL, "buffers must be 16-byte aligned");
+        return kpz_fail(c, KPZ_ENOMEM, "bound buffers too small: need %zu + %zu bytes", c->lattice_bytes, c->sl.total);
+    if (((uintptr_t)d_lattice & 15u) || ((uintptr_t)d_scratch & 15u)) return kpz_fail(c, KPZ_EINVAL, "buffers must be 16-byte aligned");
     // the device is the one that owns the buffers, whatever device is current in the calling thread
     cudaPointerAttributes al, as;
     KPZ_CUDA(c, cudaPointerGetAttributes(&al, d_lattice));
     KPZ_CUDA(c, cudaPointerGetAttributes(&as, d_scratch));
     if (al.type != cudaMemoryTypeDevice || as.type != cudaMemoryTypeDevice || al.device != as.device)
-        return fail(c, KPZ_EINVAL, "lattice and scratch must be device memory of one device");
-    if (al.device < 0 || al.device >= KPZ_MAX_DEVICES) return fail(c, KPZ_EINVAL, "device ordinal out of range");
+        return kpz_fail(c, KPZ_EINVAL, "lattice and scratch must be device memory of one device");
+    if (al.device < 0 || al.device >= KPZ_MAX_DEVICES) return kpz_fail(c, KPZ_EINVAL, "device ordinal out of range");
     c->device = al.device;
     DeviceGuard dg__(c->device);
     c->d_lattice = static_cast<uint32_t*>(d_lattice);
@@ -453,11 +332,11 @@ int32_t kpz_run(kpz_ctx* c, uint64_t mcs) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
-    if (c->mcs + mcs > 0xFFFFFFFFull) return fail(c, KPZ_EINVAL, "MCS clock would exceed 2^32-1");
+    if (c->mcs + mcs > 0xFFFFFFFFull) return kpz_fail(c, KPZ_EINVAL, "MCS clock would exceed 2^32-1");
     if (mcs == 0) return KPZ_OK;
     ResidentPlan pl{};
     const int32_t path = choose_path(c, pl);
-    if (path < 0) return fail(c, KPZ_EINVAL, "the resident path needs a power-of-two L that fits in shared memory and the default schedule");
+    if (path < 0) return kpz_fail(c, KPZ_EINVAL, "the resident path needs a lattice that fits in shared memory and the default schedule");
     if (path != KPZ_PATH_TILED) {
         rc = launch_resident(c, pl, (uint32_t)c->mcs, (uint32_t)mcs);
         if (rc != KPZ_OK) return rc;
@@ -482,14 +361,14 @@ int32_t kpz_run(kpz_ctx* c, uint64_t mcs) {
 
 int32_t kpz_set_path(kpz_ctx* c, int32_t path) {
     if (!c) return KPZ_EINVAL;
-    if (path < KPZ_PATH_AUTO || path > KPZ_PATH_RESIDENT_COOP) return fail(c, KPZ_EINVAL, "unknown path");
+    if (path < KPZ_PATH_AUTO || path > KPZ_PATH_RESIDENT) return kpz_fail(c, KPZ_EINVAL, "unknown path");
     c->path = path;
     return KPZ_OK;
 }
 
 int32_t kpz_set_schedule(kpz_ctx* c, int32_t schedule) {
     if (!c) return KPZ_EINVAL;
-    if (schedule != KPZ_SCHEDULE_COLOURS && schedule != KPZ_SCHEDULE_DEAD_BORDER) return fail(c, KPZ_EINVAL, "unknown schedule");
+    if (schedule != KPZ_SCHEDULE_COLOURS && schedule != KPZ_SCHEDULE_DEAD_BORDER) return kpz_fail(c, KPZ_EINVAL, "unknown schedule");
     c->schedule = schedule;
     return KPZ_OK;
 }
@@ -499,7 +378,7 @@ static int32_t upload_poisson_table(kpz_ctx* c);
 int32_t kpz_set_sub_sweeps(kpz_ctx* c, uint32_t K) {
     if (!c) return KPZ_EINVAL;
     const uint32_t calls = c->T * c->T / 8u;
-    if (K < 1 || K > calls || calls % K != 0) return fail(c, KPZ_EINVAL, "sub-sweeps must divide tile*tile/8");
+    if (K < 1 || K > calls || calls % K != 0) return kpz_fail(c, KPZ_EINVAL, "sub-sweeps must divide tile*tile/8");
     c->sub_sweeps = K;
     DeviceGuard dg__(c->device);
     return (c->poisson && c->bound) ? upload_poisson_table(c) : KPZ_OK;
@@ -512,7 +391,7 @@ static int32_t upload_poisson_table(kpz_ctx* c) {
     while (W * W < 144ull * lam) ++W;
     W += 16;
     const uint64_t kmin = lam > W ? lam - W : 0, kmax = lam + W, n = kmax - kmin + 1;
-    if (n > 4096) return fail(c, KPZ_EINVAL, "Poisson table too large");
+    if (n > 4096) return kpz_fail(c, KPZ_EINVAL, "Poisson table too large");
     std::vector<u128> w(n);
     w[lam - kmin] = (u128)1 << 52;
     for (uint64_t k = lam + 1; k <= kmax; ++k) w[k - kmin] = w[k - kmin - 1] * lam / k;
@@ -561,7 +440,7 @@ int32_t kpz_measure(kpz_ctx* c, int64_t* sum_h, int64_t* sum_h2, double* W2) {
         if (sum_h) { if (fits_i64(sh)) sum_h[r] = (int64_t)sh; else { sum_h[r] = 0; overflow = true; } }
         if (sum_h2) { if (fits_i64(sh2)) sum_h2[r] = (int64_t)sh2; else { sum_h2[r] = 0; overflow = true; } }
     }
-    if (overflow) return fail(c, KPZ_EOVERFLOW, "a sum does not fit int64");
+    if (overflow) return kpz_fail(c, KPZ_EOVERFLOW, "a sum does not fit int64");
     return KPZ_OK;
 }
 
@@ -569,10 +448,10 @@ int32_t kpz_run_sampled(kpz_ctx* c, const uint64_t* times, uint32_t n_times, int
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
-    if (!times || n_times == 0) return fail(c, KPZ_EINVAL, "no sampling times");
+    if (!times || n_times == 0) return kpz_fail(c, KPZ_EINVAL, "no sampling times");
     uint64_t prev = c->mcs;
     for (uint32_t i = 0; i < n_times; ++i) {
-        if (times[i] < prev || (i > 0 && times[i] == times[i - 1])) return fail(c, KPZ_EINVAL, "sampling times must increase from the current MCS clock");
+        if (times[i] < prev || (i > 0 && times[i] == times[i - 1])) return kpz_fail(c, KPZ_EINVAL, "sampling times must increase from the current MCS clock");
         prev = times[i];
     }
     int32_t worst = KPZ_OK;
@@ -588,6 +467,12 @@ int32_t kpz_run_sampled(kpz_ctx* c, const uint64_t* times, uint32_t n_times, int
 }
 
 int32_t kpz_destroy(kpz_ctx* c) {
+    if (c) {
+        DeviceGuard dg__(c->device);
+        for (cudaEvent_t e : c->events) cudaEventDestroy(e);
+        if (c->s_in) cudaStreamDestroy(c->s_in);
+        if (c->s_out) cudaStreamDestroy(c->s_out);
+    }
     delete c;
     return KPZ_OK;
 }
@@ -607,10 +492,10 @@ int32_t kpz_get_window(kpz_ctx* c, uint32_t replica, uint32_t x0, uint32_t y0, u
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
-    if (replica >= c->R || !sx || !sy || w == 0 || h == 0 || w > c->L || h > c->L) return fail(c, KPZ_EINVAL, "bad window");
+    if (replica >= c->R || !sx || !sy || w == 0 || h == 0 || w > c->L || h > c->L) return kpz_fail(c, KPZ_EINVAL, "bad window");
     const size_t n = (size_t)w * h;
     int8_t* d = nullptr;
-    if (cudaMalloc(&d, 2 * n) != cudaSuccess) { cudaGetLastError(); return fail(c, KPZ_ENOMEM, "temporary device buffer"); }
+    if (cudaMalloc(&d, 2 * n) != cudaSuccess) { cudaGetLastError(); return kpz_fail(c, KPZ_ENOMEM, "temporary device buffer"); }
     kpz::kpz_unpack_window_kernel<<<grid_for(n, 256), 256, 0, c->stream>>>(c->d_lattice, (uint64_t)c->L * c->L / 32, replica,
                                                                        c->L, c->L / 32, x0 % c->L, y0 % c->L, w, h, d, d + n);
     cudaError_t e = cudaGetLastError();
@@ -619,7 +504,7 @@ int32_t kpz_get_window(kpz_ctx* c, uint32_t replica, uint32_t x0, uint32_t y0, u
     if (e == cudaSuccess) e = cudaMemcpyAsync(sy, d + n, n, cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     cudaFree(d);
-    if (e != cudaSuccess) return fail(c, KPZ_ECUDA, "get_window: %s", cudaGetErrorString(e));
+    if (e != cudaSuccess) return kpz_fail(c, KPZ_ECUDA, "get_window: %s", cudaGetErrorString(e));
     return KPZ_OK;
 }
 
@@ -632,10 +517,10 @@ int32_t kpz_set_slopes(kpz_ctx* c, uint32_t replica, const int8_t* sx, const int
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
-    if (replica >= c->R || !sx || !sy) return fail(c, KPZ_EINVAL, "bad argument");
+    if (replica >= c->R || !sx || !sy) return kpz_fail(c, KPZ_EINVAL, "bad argument");
     const size_t n = (size_t)c->L * c->L;
     int8_t* d = nullptr;
-    if (cudaMalloc(&d, 2 * n) != cudaSuccess) { cudaGetLastError(); return fail(c, KPZ_ENOMEM, "temporary device buffer"); }
+    if (cudaMalloc(&d, 2 * n) != cudaSuccess) { cudaGetLastError(); return kpz_fail(c, KPZ_ENOMEM, "temporary device buffer"); }
     int* flags = reinterpret_cast<int*>(c->d_scratch + c->sl.misc + 8);
     int hflags = 0;
     cudaError_t e = cudaMemcpyAsync(d, sx, n, cudaMemcpyHostToDevice, c->stream);
@@ -659,9 +544,9 @@ int32_t kpz_set_slopes(kpz_ctx* c, uint32_t replica, const int8_t* sx, const int
         if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     }
     cudaFree(d);
-    if (e != cudaSuccess) return fail(c, KPZ_ECUDA, "set_slopes: %s", cudaGetErrorString(e));
-    if (hflags & 1) return fail(c, KPZ_EINVAL, "slopes must be +1 or -1");
-    if (hflags) return fail(c, KPZ_ESTATE, "state is not curl-free with zero tilt (flags %d)", hflags);
+    if (e != cudaSuccess) return kpz_fail(c, KPZ_ECUDA, "set_slopes: %s", cudaGetErrorString(e));
+    if (hflags & 1) return kpz_fail(c, KPZ_EINVAL, "slopes must be +1 or -1");
+    if (hflags) return kpz_fail(c, KPZ_ESTATE, "state is not curl-free with zero tilt (flags %d)", hflags);
     return KPZ_OK;
 }
 
@@ -669,7 +554,7 @@ int32_t kpz_state_hash(kpz_ctx* c, uint32_t replica, uint64_t* out) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
-    if (replica >= c->R || !out) return fail(c, KPZ_EINVAL, "bad argument");
+    if (replica >= c->R || !out) return kpz_fail(c, KPZ_EINVAL, "bad argument");
     unsigned long long* acc = reinterpret_cast<unsigned long long*>(c->d_scratch + c->sl.misc);
     const uint64_t plane_words = (uint64_t)c->L * c->L / 32;
     KPZ_CUDA(c, cudaMemsetAsync(acc, 0, 8, c->stream));
@@ -688,7 +573,7 @@ int32_t kpz_counters(kpz_ctx* c, uint32_t replica, uint64_t* attempts, uint64_t*
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
-    if (replica >= c->R) return fail(c, KPZ_EINVAL, "replica out of range");
+    if (replica >= c->R) return kpz_fail(c, KPZ_EINVAL, "replica out of range");
     unsigned long long st[4];
     KPZ_CUDA(c, cudaMemcpyAsync(st, c->d_scratch + c->sl.stats + (size_t)replica * 32, 32, cudaMemcpyDeviceToHost, c->stream));
     KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -704,7 +589,7 @@ int32_t kpz_export_packed(kpz_ctx* c, void* host_dst, size_t bytes) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
-    if (!host_dst || bytes < c->lattice_bytes) return fail(c, KPZ_EINVAL, "host buffer too small");
+    if (!host_dst || bytes < c->lattice_bytes) return kpz_fail(c, KPZ_EINVAL, "host buffer too small");
     KPZ_CUDA(c, cudaMemcpyAsync(host_dst, c->d_lattice, c->lattice_bytes, cudaMemcpyDeviceToHost, c->stream));
     KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
     return KPZ_OK;
@@ -714,7 +599,7 @@ int32_t kpz_import_packed(kpz_ctx* c, const void* host_src, size_t bytes, const 
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
-    if (!host_src || bytes < c->lattice_bytes || mcs > 0xFFFFFFFFull) return fail(c, KPZ_EINVAL, "bad argument");
+    if (!host_src || bytes < c->lattice_bytes || mcs > 0xFFFFFFFFull) return kpz_fail(c, KPZ_EINVAL, "bad argument");
     KPZ_CUDA(c, cudaMemcpyAsync(c->d_lattice, host_src, c->lattice_bytes, cudaMemcpyHostToDevice, c->stream));
     std::vector<unsigned long long> st((size_t)c->R * 4, 0ull);
     KPZ_CUDA(c, cudaMemcpyAsync(st.data(), c->d_scratch + c->sl.stats, (size_t)c->R * 32, cudaMemcpyDeviceToHost, c->stream));
@@ -750,16 +635,17 @@ int32_t kpz_step_host(kpz_ctx* c, void* host_lattice, size_t bytes, int64_t* h00
 
 namespace {
 
-// streams and events of one kpz_pipeline_host call, released on every return path
-struct PipelineResources {
-    cudaStream_t s_in = nullptr, s_out = nullptr;
-    std::vector<cudaEvent_t> ev;
-    ~PipelineResources() {
-        for (cudaEvent_t e : ev) if (e) cudaEventDestroy(e);
-        if (s_in) cudaStreamDestroy(s_in);
-        if (s_out) cudaStreamDestroy(s_out);
+// copy streams and events of kpz_pipeline_host: created on the first call, kept in the handle, released by kpz_destroy
+int32_t pipeline_resources(kpz_ctx* c, size_t n_events) {
+    if (!c->s_in) KPZ_CUDA(c, cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking));
+    if (!c->s_out) KPZ_CUDA(c, cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking));
+    while (c->events.size() < n_events) {
+        cudaEvent_t e = nullptr;
+        KPZ_CUDA(c, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        c->events.push_back(e);
     }
-};
+    return KPZ_OK;
+}
 
 // overwrite the tracked h(0,0) of every replica (stats[r][2]) and clear the S7 attempt counter, on the bound stream
 int32_t set_h00(kpz_ctx* c, const int64_t* h00) {
@@ -790,19 +676,21 @@ int32_t kpz_pipeline_host(kpz_ctx* c, void* device_lattice2, size_t device_latti
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
     if (!device_lattice2 || device_lattice2_bytes < c->lattice_bytes || ((uintptr_t)device_lattice2 & 15u))
-        return fail(c, KPZ_EINVAL, "second device lattice missing, too small or not 16-byte aligned");
+        return kpz_fail(c, KPZ_EINVAL, "second device lattice missing, too small or not 16-byte aligned");
     if (n_lanes == 0 || n_rounds == 0 || !host_lattices || !mcs_start || bytes < c->lattice_bytes)
-        return fail(c, KPZ_EINVAL, "bad argument");
+        return kpz_fail(c, KPZ_EINVAL, "bad argument");
     for (uint32_t l = 0; l < n_lanes; ++l) {
-        if (!host_lattices[l]) return fail(c, KPZ_EINVAL, "NULL host lattice");
-        if (mcs_start[l] + (uint64_t)n_rounds * mcs > 0xFFFFFFFFull) return fail(c, KPZ_EINVAL, "MCS clock would exceed 2^32-1");
+        if (!host_lattices[l]) return kpz_fail(c, KPZ_EINVAL, "NULL host lattice");
+        if (mcs_start[l] + (uint64_t)n_rounds * mcs > 0xFFFFFFFFull) return kpz_fail(c, KPZ_EINVAL, "MCS clock would exceed 2^32-1");
     }
     const uint64_t B = (uint64_t)n_lanes * n_rounds;   // batches, b = round * n_lanes + lane
-    PipelineResources res;
-    KPZ_CUDA(c, cudaStreamCreateWithFlags(&res.s_in, cudaStreamNonBlocking));
-    KPZ_CUDA(c, cudaStreamCreateWithFlags(&res.s_out, cudaStreamNonBlocking));
-    res.ev.assign((size_t)B * 2, nullptr);               // per batch: copied in, copied out
-    for (cudaEvent_t& e : res.ev) KPZ_CUDA(c, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    // per batch two events (copied in, copied out); events are reused round-robin: a batch only ever waits for
+    // batches at most max(2, n_lanes) behind it, so a window of that many (+2) batches suffices
+    const uint64_t EW = (n_lanes > 2 ? n_lanes : 2) + 2;     // batches in the event window
+    rc = pipeline_resources(c, (size_t)EW * 2);
+    if (rc != KPZ_OK) return rc;
+    struct { cudaStream_t s_in, s_out; cudaEvent_t* ev; uint64_t EW; cudaEvent_t& in(uint64_t b) { return ev[2 * (b % EW)]; }
+             cudaEvent_t& out(uint64_t b) { return ev[2 * (b % EW) + 1]; } } res{c->s_in, c->s_out, c->events.data(), EW};
     uint32_t* const dbuf[2] = {c->d_lattice, static_cast<uint32_t*>(device_lattice2)};
     std::vector<int64_t> h00((size_t)n_lanes * c->R, 0);
     if (h00_inout) std::memcpy(h00.data(), h00_inout, h00.size() * sizeof(int64_t));
@@ -811,10 +699,10 @@ int32_t kpz_pipeline_host(kpz_ctx* c, void* device_lattice2, size_t device_latti
     // host->device copy of batch b: its device slot must have been copied out (batch b-2), and so must the last
     // batch of the same lane (b - n_lanes), whose output is this batch's input
     auto enqueue_in = [&](uint64_t b) -> int32_t {
-        if (b >= 2) KPZ_CUDA(c, cudaStreamWaitEvent(res.s_in, res.ev[2 * (b - 2) + 1], 0));
-        if (b >= n_lanes) KPZ_CUDA(c, cudaStreamWaitEvent(res.s_in, res.ev[2 * (b - n_lanes) + 1], 0));
+        if (b >= 2) KPZ_CUDA(c, cudaStreamWaitEvent(res.s_in, res.out(b - 2), 0));
+        if (b >= n_lanes) KPZ_CUDA(c, cudaStreamWaitEvent(res.s_in, res.out(b - n_lanes), 0));
         KPZ_CUDA(c, cudaMemcpyAsync(dbuf[b & 1], host_lattices[b % n_lanes], c->lattice_bytes, cudaMemcpyHostToDevice, res.s_in));
-        KPZ_CUDA(c, cudaEventRecord(res.ev[2 * b], res.s_in));
+        KPZ_CUDA(c, cudaEventRecord(res.in(b), res.s_in));
         return KPZ_OK;
     };
 
@@ -833,7 +721,7 @@ int32_t kpz_pipeline_host(kpz_ctx* c, void* device_lattice2, size_t device_latti
             c->d_lattice = dbuf[b & 1];
             c->mcs = clock[lane];
             c->attempts_base = clock[lane] * (uint64_t)c->L * c->L;
-            KPZ_CUDA(c, cudaStreamWaitEvent(c->stream, res.ev[2 * b], 0));
+            KPZ_CUDA(c, cudaStreamWaitEvent(c->stream, res.in(b), 0));
             if ((r = kpz_run(c, mcs)) != KPZ_OK) return r;
             const size_t o = (size_t)b * c->R;
             r = kpz_measure(c, sum_h ? sum_h + o : nullptr, sum_h2 ? sum_h2 + o : nullptr, W2 ? W2 + o : nullptr);
@@ -844,7 +732,7 @@ int32_t kpz_pipeline_host(kpz_ctx* c, void* device_lattice2, size_t device_latti
             clock[lane] += mcs;
             if (b + 1 < B && (r = set_h00(c, &h00[(size_t)((b + 1) % n_lanes) * c->R])) != KPZ_OK) return r;
             KPZ_CUDA(c, cudaMemcpyAsync(host_lattices[lane], dbuf[b & 1], c->lattice_bytes, cudaMemcpyDeviceToHost, res.s_out));
-            KPZ_CUDA(c, cudaEventRecord(res.ev[2 * b + 1], res.s_out));
+            KPZ_CUDA(c, cudaEventRecord(res.out(b), res.s_out));
             if (n_lanes == 1 && b + 1 < B && (r = enqueue_in(b + 1)) != KPZ_OK) return r;
         }
         KPZ_CUDA(c, cudaStreamSynchronize(res.s_out));
@@ -866,7 +754,7 @@ static int32_t run_profiles(kpz_ctx* c, uint32_t replica, bool with_fft, long lo
     const uint32_t L = c->L, W = L / 32;
     uint32_t logL = 0;
     while ((1u << logL) < L) ++logL;
-    if (with_fft && (1u << logL) != L) return fail(c, KPZ_EINVAL, "the power spectrum needs L to be a power of two");
+    if (with_fft && (1u << logL) != L) return kpz_fail(c, KPZ_EINVAL, "the power spectrum needs L to be a power of two");
     std::vector<i128> S1, S2;
     std::vector<long long> h00;
     int32_t rc = measure_relative(c, S1, S2, h00, true, replica);
@@ -897,7 +785,7 @@ int32_t kpz_profiles(kpz_ctx* c, uint32_t replica, int64_t* col_sums, int64_t* r
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
-    if (replica >= c->R) return fail(c, KPZ_EINVAL, "replica out of range");
+    if (replica >= c->R) return kpz_fail(c, KPZ_EINVAL, "replica out of range");
     long long h00 = 0;
     rc = run_profiles(c, replica, false, &h00);
     if (rc != KPZ_OK) return rc;
@@ -916,7 +804,7 @@ int32_t kpz_power_spectrum(kpz_ctx* c, uint32_t replica, double* S, double* Sx, 
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
-    if (replica >= c->R) return fail(c, KPZ_EINVAL, "replica out of range");
+    if (replica >= c->R) return kpz_fail(c, KPZ_EINVAL, "replica out of range");
     long long h00 = 0;
     rc = run_profiles(c, replica, true, &h00);
     if (rc != KPZ_OK) return rc;
@@ -931,6 +819,43 @@ int32_t kpz_power_spectrum(kpz_ctx* c, uint32_t replica, double* S, double* Sx, 
 int32_t kpz_launch_count(const kpz_ctx* c, uint64_t* out) {
     if (!c || !out) return KPZ_EINVAL;
     *out = c->launches;
+    return KPZ_OK;
+}
+
+int32_t kpz_measure_peaks(double* out, uint32_t n) {
+    if (!out || n < KPZ_N_PEAKS) return KPZ_EINVAL;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return KPZ_ECUDA;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) return KPZ_ECUDA;
+    const uint32_t blocks = (uint32_t)sms * 8u;              // 8 CTAs of 256 threads per SM: every warp slot busy
+    uint32_t* sink = nullptr;
+    unsigned long long* ticks = nullptr;
+    if (cudaMalloc(&sink, blocks * sizeof(uint32_t)) != cudaSuccess) { cudaGetLastError(); return KPZ_ECUDA; }
+    if (cudaMalloc(&ticks, 8) != cudaSuccess) { cudaGetLastError(); cudaFree(sink); return KPZ_ECUDA; }
+    const uint32_t iters = 2048;
+    const double lanes = (double)blocks * 256.0 * iters * kpz::PEAK_UNROLL;        // lane-instructions of the measured kind
+    float ms[7] = {0, 0, 0, 0, 0, 0, 0};
+    cudaError_t e = run_peak<kpz::PEAK_LOP3>(blocks, iters, sink, ticks, &ms[0]);
+    unsigned long long hticks = 0;
+    if (e == cudaSuccess) e = cudaMemcpy(&hticks, ticks, 8, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = run_peak<kpz::PEAK_SHF>(blocks, iters, sink, ticks, &ms[1]);
+    if (e == cudaSuccess) e = run_peak<kpz::PEAK_IMAD>(blocks, iters, sink, ticks, &ms[2]);
+    if (e == cudaSuccess) e = run_peak<kpz::PEAK_IMAD_WIDE>(blocks, iters, sink, ticks, &ms[3]);
+    if (e == cudaSuccess) e = run_peak<kpz::PEAK_LDS>(blocks, iters, sink, ticks, &ms[4]);
+    if (e == cudaSuccess) e = run_peak<kpz::PEAK_ATOMS>(blocks, iters, sink, ticks, &ms[5]);
+    if (e == cudaSuccess) e = run_peak<kpz::PEAK_MIX>(blocks, iters / 4, sink, ticks, &ms[6]);
+    cudaFree(sink);
+    cudaFree(ticks);
+    if (e != cudaSuccess) return KPZ_ECUDA;
+    out[0] = (double)hticks / (ms[0] * 1e-3);          // SM clock while the LOP3 kernel ran (block 0's ticks / event time)
+    out[1] = lanes / (ms[0] * 1e-3);                   // LOP3 lane-ops/s
+    out[2] = lanes / (ms[1] * 1e-3);                   // SHF lane-ops/s
+    out[3] = lanes / (ms[2] * 1e-3);                   // IMAD lane-ops/s
+    out[4] = lanes / (ms[3] * 1e-3);                   // IMAD.WIDE lane-ops/s (one LOP3 rides along each)
+    out[5] = lanes * 4.0 / (ms[4] * 1e-3);             // LDS.32 bytes/s, every lane in its own bank
+    out[6] = lanes / (ms[5] * 1e-3);                   // shared-memory XOR reductions (lane-ops/s)
+    out[7] = lanes / 4.0 / (ms[6] * 1e-3);             // attempts/s of the bare instruction mix of one p = 1 attempt, no chain
+    out[8] = (double)sms;
     return KPZ_OK;
 }
 

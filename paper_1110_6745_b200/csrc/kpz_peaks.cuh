@@ -1,0 +1,81 @@
+// kpz_peaks.cuh -- micro-benchmarks of the pipes that bound kpz_update_kernel.
+//
+// MEASURED_PEAKS.json carries HBM bandwidth and bf16 tensor throughput only; the update kernel is bound by the
+// integer ALU pipe (LOP3 / SHF / LEA) and by the shared-memory data pipe (LDS / ATOMS wavefronts), so their peaks
+// are measured here, on the box, by kernels that do nothing but issue one kind of instruction from every warp
+// slot of every SM.  Each kernel runs ITER iterations of an unrolled body of independent chains (eight registers,
+// so that neither latency nor the register file limits the issue rate); its rate is instructions x 32 lanes /
+// CUDA-event time.  The SM clock during the measurement is read back as clock64() ticks / event time.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace kpz {
+
+enum PeakKind { PEAK_LOP3 = 0, PEAK_SHF = 1, PEAK_IMAD = 2, PEAK_IMAD_WIDE = 3, PEAK_LDS = 4, PEAK_ATOMS = 5, PEAK_MIX = 6 };
+
+constexpr int PEAK_UNROLL = 64;      // instructions of the measured kind per loop iteration and chain group
+
+template <int KIND>
+__global__ void __launch_bounds__(256) kpz_peak_kernel(uint32_t iters, uint32_t seed, uint32_t* __restrict__ sink,
+                                                       unsigned long long* __restrict__ ticks) {
+    __shared__ uint32_t sm[32 * 64 + 256];
+    uint32_t r[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) r[k] = seed * (2u * k + 1u) + threadIdx.x;
+    for (uint32_t i = threadIdx.x; i < 32 * 64 + 256; i += blockDim.x) sm[i] = i * seed;
+    __syncthreads();
+    // word w of lane t at sm[w * 32 + lane]: every lane in its own bank, as in the update kernel
+    uint32_t* mine = sm + (threadIdx.x & 31u);
+    const long long t0 = clock64();
+#pragma unroll 1
+    for (uint32_t it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int j = 0; j < PEAK_UNROLL / 8; ++j) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                if (KIND == PEAK_LOP3) {
+                    asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(r[k]) : "r"(r[(k + 1) & 7]), "r"(seed));
+                } else if (KIND == PEAK_SHF) {
+                    asm volatile("shf.l.wrap.b32 %0, %0, %1, 7;" : "+r"(r[k]) : "r"(r[(k + 3) & 7]));
+                } else if (KIND == PEAK_IMAD) {
+                    asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(r[k]) : "r"(seed), "r"(r[(k + 1) & 7]));
+                } else if (KIND == PEAK_IMAD_WIDE) {
+                    unsigned long long w;
+                    asm volatile("mul.wide.u32 %0, %1, %2;" : "=l"(w) : "r"(r[k]), "r"(0xD2511F53u));
+                    r[k] = (uint32_t)(w >> 32) ^ (uint32_t)w;       // one LOP3 per multiply rides along (Philox does the same)
+                } else if (KIND == PEAK_LDS) {
+                    uint32_t v;
+                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(mine + 32 * ((j * 8 + k) & 63))));
+                    r[k] ^= v;
+                } else if (KIND == PEAK_ATOMS) {
+                    asm volatile("red.shared.xor.b32 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(mine + 32 * ((j * 8 + k) & 63))), "r"(r[k]) : "memory");
+                } else {
+                    // the instruction mix of one p = 1 attempt: 5 LDS, 2 SHF, 3 LOP3, 1 ATOMS on private banks
+                    uint32_t a, b, c, d, e;
+                    const uint32_t base = (uint32_t)__cvta_generic_to_shared(mine + 32 * ((r[k] >> 27) + 2 * k));
+                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(a) : "r"(base));
+                    asm volatile("ld.shared.u32 %0, [%1+128];" : "=r"(b) : "r"(base));
+                    asm volatile("ld.shared.u32 %0, [%1+256];" : "=r"(c) : "r"(base));
+                    asm volatile("ld.shared.u32 %0, [%1+384];" : "=r"(d) : "r"(base));
+                    asm volatile("ld.shared.u32 %0, [%1+512];" : "=r"(e) : "r"(base));
+                    const uint32_t wl = __funnelshift_l(a, b, 1), wr = __funnelshift_r(b, c, 1);
+                    uint32_t t1, t2, md;
+                    asm volatile("lop3.b32 %0, %1, %2, %3, 0xdb;" : "=r"(t1) : "r"(b), "r"(wl), "r"(wr));
+                    asm volatile("lop3.b32 %0, %1, %2, %3, 0xbd;" : "=r"(t2) : "r"(b), "r"(d), "r"(e));
+                    asm volatile("lop3.b32 %0, %1, %2, %3, 0x10;" : "=r"(md) : "r"(r[k]), "r"(t1), "r"(t2));
+                    asm volatile("red.shared.xor.b32 [%0+128], %1;" ::"r"(base), "r"(md & 1u) : "memory");
+                    r[k] = r[k] * 0x9E3779B9u + md;
+                }
+            }
+        }
+    }
+    const long long t1 = clock64();
+    uint32_t acc = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) acc ^= r[k];
+    if (acc == 0x12345678u) sink[blockIdx.x] = acc + sm[threadIdx.x];      // keeps the chains alive, never true in practice
+    if (blockIdx.x == 0 && threadIdx.x == 0) ticks[0] = (unsigned long long)(t1 - t0);
+}
+
+}  // namespace kpz

@@ -22,11 +22,24 @@ def test_reference_arm_prints_one_json_line_with_the_contract_keys():
     assert "config3" in d["config"]["workload"]
 
 
-def test_roofline_constants_match_design():
+def test_algorithmic_units_follow_from_the_method():
+    """What the mathematics fixes about the roofline inputs: config 3 of BASELINE.json, one launch of the tiled update
+    kernel = one colour = L^2/4 attempted updates, each 2-bit site read once and written once per MCS = L^2/8
+    bytes per launch, five 32-bit shared-memory loads and one XOR reduction per attempt, one sigma_y bit per site for
+    the measurement (eq. 3 walks plane Y only)."""
     sys.path.insert(0, str(ROOT))
     import bench
-    assert bench.WORKLOAD == dict(L=1 << 17, tile=64, p=1.0, q=0.0, seed=42)      # BASELINE config 3
-    assert bench.MCS_PER_STEP * 10 == 100                                         # default K = 10 steps = 100 MCS
-    assert bench.ALG_BYTES_PER_UPDATE == 0.5 and bench.ALG_ALU_OPS_PER_UPDATE == 11.5
-    design = (ROOT / "DESIGN.md").read_text()
-    assert "**11.5**" in design and "18.6 T lane-ops/s" in design
+    base = json.loads((ROOT / "BASELINE.json").read_text())
+    assert "2^17" in base["configs"][2] and "tile 64" in base["configs"][2] and "seed 42" in base["configs"][2]
+    assert bench.WORKLOAD == dict(L=1 << 17, tile=64, p=1.0, q=0.0, seed=42)
+    assert bench.CONFIGS[3]["mcs_per_step"] * bench.CONFIGS[3]["steps"] == 100          # "100 MCS timed"
+    L = bench.WORKLOAD["L"]
+    updates_per_launch = L * L // 4
+    assert updates_per_launch == 2 ** 32
+    assert bench.ALG_BYTES_PER_UPDATE * updates_per_launch == L * L / 8                  # 2 bits in + 2 bits out per site and MCS, / 4 launches
+    assert 4 * bench.ALG_BYTES_PER_UPDATE * updates_per_launch == 2 * (L * L * 2 / 8)    # = the packed lattice read and written once per MCS
+    assert bench.ALG_SMEM_BYTES_PER_UPDATE == (5 + 1) * 4
+    assert bench.ALG_BYTES_PER_SITE_MEASURE * 8 == 1
+    for n, c in bench.CONFIGS.items():                                                   # every config is a valid handle
+        assert c["L"] % (2 * c["tile"]) == 0 and c["L"] % 32 == 0 and 0 <= c["q"] <= c["p"] <= 1
+    assert bench.CONFIGS[4]["replicas"] == 1024 and bench.CONFIGS[5]["L"] == 1 << 19

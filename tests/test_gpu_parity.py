@@ -167,7 +167,7 @@ def test_update_parity_every_mcs(pkg, L, T, p, q, seed, n):
         assert k.state_hash() == o.state_hash()
 
 
-@pytest.mark.parametrize("path", ["resident", "resident_coop", "auto"])
+@pytest.mark.parametrize("path", ["resident", "auto"])
 @pytest.mark.parametrize("L,T,p,q,seed,R,n", [
     (32, 4, 1.0, 0.0, 61, 1, 5),           # one word per row, 16 steps per tile: half a warp batch
     (32, 4, 0.75, 0.25, 62, 7, 4),
@@ -180,10 +180,12 @@ def test_update_parity_every_mcs(pkg, L, T, p, q, seed, n):
     (256, 64, 0.75, 0.25, 3, 1, 3),
     (512, 16, 1.0, 0.0, 67, 1, 2),
     (512, 32, 0.6, 0.1, 68, 2, 2),
+    (96, 16, 0.5, 0.5, 69, 3, 3),          # L not a power of two
+    (384, 64, 1.0, 0.0, 70, 1, 2),
 ])
 def test_resident_paths_parity(pkg, path, L, T, p, q, seed, R, n):
-    """Lattice-resident kernels (kpz_resident_kernel: one thread per tile / one warp per tile, whole lattice in shared
-    memory, n MCS per launch): state, sums, counters after every MCS, then n more MCS in ONE launch."""
+    """Lattice-resident kernel (kpz_resident_kernel: the packed lattices of a CTA's replicas in shared memory, all MCS
+    of a call in one launch): state, sums, counters after every MCS, then n more MCS in ONE launch."""
     k = pkg.KPZ(L, p, q, T, seed, n_replicas=R)
     k.set_path(path)
     k.init_flat()
@@ -217,7 +219,7 @@ def test_resident_paths_parity(pkg, path, L, T, p, q, seed, R, n):
 
 
 def test_resident_path_is_refused_when_it_cannot_hold_the_lattice(pkg):
-    for (L, T, path) in ((96, 16, "resident"), (2048, 16, "resident"), (1024, 64, "resident_coop")):
+    for (L, T, path) in ((2048, 16, "resident"), (1024, 64, "resident")):
         k = pkg.KPZ(L, 1.0, 0.0, T, 1)
         k.set_path(path)
         k.init_flat()
