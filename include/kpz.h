@@ -210,7 +210,10 @@ int32_t kpz_profiles(kpz_ctx* ctx, uint32_t replica, int64_t* col_sums, int64_t*
  * lattice axes, k = 2 pi n / L, n = 0 .. L/2:  Sx[n] = S(k,0), Sy[n] = S(0,k) and their average S[n] ("averaging
  * over x and y directions").  S[0] = 0.  HOST out-arrays of length L/2 + 1 (any may be NULL); one replica,
  * one time: ensemble averages are the caller's sum.  fp64 radix-2 FFT of the two integer profiles on the device.
- * L must be a power of two (KPZ_EINVAL otherwise).  Synchronises.  Does not modify the lattice. */
+ * L must be a power of two (KPZ_EINVAL otherwise).  Synchronises.  Does not modify the lattice.
+ * Note: the domain decomposition leaves an imprint on S(k) (R18): with the default schedule, narrow peaks
+ * at the mode numbers n = (2j+1) L / (2 tile) and n = L/4, a decade above the scaling window 0.002 < k < 0.1 of P:137;
+ * kpz_set_sub_sweeps(K >= 2) removes them. */
 int32_t kpz_power_spectrum(kpz_ctx* ctx, uint32_t replica, double* S, double* Sx, double* Sy);
 
 /* Number of kernels this handle has launched since creation (for bench.py "gpu_launches"). */
@@ -219,7 +222,7 @@ int32_t kpz_launch_count(const kpz_ctx* ctx, uint64_t* out);
 /* Pipe micro-benchmarks for the roofline of the update kernel (MEASURED_PEAKS.json has no
  * integer or shared-memory peak).  Runs, on the CURRENT device, kernels that only issue one kind of instruction from
  * every warp slot of every SM and writes KPZ_N_PEAKS doubles to the HOST array `out` (n >= KPZ_N_PEAKS):
- *   [0] SM clock in Hz during the run (clock64 ticks / CUDA-event time)
+ *   [0] SM clock in Hz during the run (clock64 ticks / globaltimer nanoseconds of one thread)
  *   [1] LOP3, [2] SHF, [3] IMAD, [4] IMAD.WIDE throughput in lane-operations/s (32 per warp instruction)
  *   [5] shared-memory LDS.32 bytes/s with every lane in its own bank (the tile layout of the update kernel)
  *   [6] shared-memory XOR reductions (ATOMS / RED) in lane-operations/s

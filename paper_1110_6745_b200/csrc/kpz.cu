@@ -831,13 +831,13 @@ int32_t kpz_measure_peaks(double* out, uint32_t n) {
     uint32_t* sink = nullptr;
     unsigned long long* ticks = nullptr;
     if (cudaMalloc(&sink, blocks * sizeof(uint32_t)) != cudaSuccess) { cudaGetLastError(); return KPZ_ECUDA; }
-    if (cudaMalloc(&ticks, 8) != cudaSuccess) { cudaGetLastError(); cudaFree(sink); return KPZ_ECUDA; }
+    if (cudaMalloc(&ticks, 16) != cudaSuccess) { cudaGetLastError(); cudaFree(sink); return KPZ_ECUDA; }
     const uint32_t iters = 2048;
     const double lanes = (double)blocks * 256.0 * iters * kpz::PEAK_UNROLL;        // lane-instructions of the measured kind
     float ms[7] = {0, 0, 0, 0, 0, 0, 0};
     cudaError_t e = run_peak<kpz::PEAK_LOP3>(blocks, iters, sink, ticks, &ms[0]);
-    unsigned long long hticks = 0;
-    if (e == cudaSuccess) e = cudaMemcpy(&hticks, ticks, 8, cudaMemcpyDeviceToHost);
+    unsigned long long hticks[2] = {0, 1};
+    if (e == cudaSuccess) e = cudaMemcpy(hticks, ticks, 16, cudaMemcpyDeviceToHost);
     if (e == cudaSuccess) e = run_peak<kpz::PEAK_SHF>(blocks, iters, sink, ticks, &ms[1]);
     if (e == cudaSuccess) e = run_peak<kpz::PEAK_IMAD>(blocks, iters, sink, ticks, &ms[2]);
     if (e == cudaSuccess) e = run_peak<kpz::PEAK_IMAD_WIDE>(blocks, iters, sink, ticks, &ms[3]);
@@ -847,7 +847,7 @@ int32_t kpz_measure_peaks(double* out, uint32_t n) {
     cudaFree(sink);
     cudaFree(ticks);
     if (e != cudaSuccess) return KPZ_ECUDA;
-    out[0] = (double)hticks / (ms[0] * 1e-3);          // SM clock while the LOP3 kernel ran (block 0's ticks / event time)
+    out[0] = (double)hticks[0] / ((double)(hticks[1] ? hticks[1] : 1) * 1e-9);   // SM clock while the LOP3 kernel ran
     out[1] = lanes / (ms[0] * 1e-3);                   // LOP3 lane-ops/s
     out[2] = lanes / (ms[1] * 1e-3);                   // SHF lane-ops/s
     out[3] = lanes / (ms[2] * 1e-3);                   // IMAD lane-ops/s

@@ -5,7 +5,7 @@
 // are measured here, on the box, by kernels that do nothing but issue one kind of instruction from every warp
 // slot of every SM.  Each kernel runs ITER iterations of an unrolled body of independent chains (eight registers,
 // so that neither latency nor the register file limits the issue rate); its rate is instructions x 32 lanes /
-// CUDA-event time.  The SM clock during the measurement is read back as clock64() ticks / event time.
+// CUDA-event time.  The SM clock during the measurement is read back as clock64() ticks / globaltimer nanoseconds of one thread.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -27,6 +27,10 @@ __global__ void __launch_bounds__(256) kpz_peak_kernel(uint32_t iters, uint32_t 
     __syncthreads();
     // word w of lane t at sm[w * 32 + lane]: every lane in its own bank, as in the update kernel
     uint32_t* mine = sm + (threadIdx.x & 31u);
+    // SM clock = clock64 ticks per globaltimer nanosecond of the same thread (independent of how the scheduler
+    // interleaves the CTAs of an SM)
+    unsigned long long g0, g1;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0));
     const long long t0 = clock64();
 #pragma unroll 1
     for (uint32_t it = 0; it < iters; ++it) {
@@ -46,7 +50,8 @@ __global__ void __launch_bounds__(256) kpz_peak_kernel(uint32_t iters, uint32_t 
                     r[k] = (uint32_t)(w >> 32) ^ (uint32_t)w;       // one LOP3 per multiply rides along (Philox does the same)
                 } else if (KIND == PEAK_LDS) {
                     uint32_t v;
-                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(mine + 32 * ((j * 8 + k) & 63))));
+                    // ld.volatile: ptxas would hoist a plain load from a loop-invariant address out of the loop
+                    asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(mine + 32 * ((j * 8 + k) & 63))) : "memory");
                     r[k] ^= v;
                 } else if (KIND == PEAK_ATOMS) {
                     asm volatile("red.shared.xor.b32 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(mine + 32 * ((j * 8 + k) & 63))), "r"(r[k]) : "memory");
@@ -71,11 +76,15 @@ __global__ void __launch_bounds__(256) kpz_peak_kernel(uint32_t iters, uint32_t 
         }
     }
     const long long t1 = clock64();
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
     uint32_t acc = 0;
 #pragma unroll
     for (int k = 0; k < 8; ++k) acc ^= r[k];
     if (acc == 0x12345678u) sink[blockIdx.x] = acc + sm[threadIdx.x];      // keeps the chains alive, never true in practice
-    if (blockIdx.x == 0 && threadIdx.x == 0) ticks[0] = (unsigned long long)(t1 - t0);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        ticks[0] = (unsigned long long)(t1 - t0);
+        ticks[1] = g1 - g0;
+    }
 }
 
 }  // namespace kpz

@@ -50,6 +50,8 @@ def run(L, replicas, tile=16, p=1.0, q=0.0, seed=4, t_end=None, samples=100, spe
             S = np.mean([k.power_spectrum(r)[0] for r in range(n)], axis=0)
             out["spectrum_replicas"] = n
             out["S_k"] = S.tolist()
+            # the schedule's imprint on S(k) (R18): the affected modes, each beside its neighbourhood
+            out["schedule_peaks"] = schedule_peaks(S, L, tile) if L >= 8 * tile else []
         return out
     finally:
         k.close()
