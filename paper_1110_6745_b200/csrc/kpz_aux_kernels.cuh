@@ -90,10 +90,10 @@ __global__ void __launch_bounds__(128) kpz_column_chunk_kernel(const uint32_t* _
                                                                uint64_t plane_words, uint32_t L, uint32_t W,
                                                                uint32_t rows_per_chunk, int32_t* __restrict__ cS0,
                                                                int32_t* __restrict__ cS1, int32_t* __restrict__ cS2) {
-    // (S0 & 0xFF) | (S1 & 0xFF) << 8 | S2 << 16 for each byte value, replicated once per shared-memory bank: lane t
-    // reads lut[32 * byte + t], so the 32 independent look-ups of a warp never collide (one 256-entry copy cost
-    // 1.6e8 bank conflicts per measurement at L = 2^17, profiles/r01_v4.md)
-    __shared__ uint32_t lut[256 * 32];
+    // One 256-entry copy for the whole CTA.  (A copy per bank, lut[32 * byte + lane], removes the 1.6e8 bank
+    // conflicts of a measurement at L = 2^17 but costs an index shift and 32 KB per CTA: 1.76 ms against 1.54 ms,
+    // the kernel is bound by the ALU pipe at 70 %, not by the table -- measured in round 2 and dropped.)
+    __shared__ uint32_t lut[256];      // (S0 & 0xFF) | (S1 & 0xFF) << 8 | S2 << 16
     for (uint32_t b = threadIdx.x; b < 256u; b += blockDim.x) {
         int l = 0, s1 = 0, s2 = 0;
         for (int k = 0; k < 8; ++k) {
@@ -101,12 +101,9 @@ __global__ void __launch_bounds__(128) kpz_column_chunk_kernel(const uint32_t* _
             s1 += l;
             s2 += l * l;
         }
-        const uint32_t e = ((uint32_t)l & 0xFFu) | (((uint32_t)s1 & 0xFFu) << 8) | ((uint32_t)s2 << 16);
-#pragma unroll
-        for (int t = 0; t < 32; ++t) lut[32u * b + t] = e;
+        lut[b] = ((uint32_t)l & 0xFFu) | (((uint32_t)s1 & 0xFFu) << 8) | ((uint32_t)s2 << 16);
     }
     __syncthreads();
-    const uint32_t* mylut = lut + (threadIdx.x & 31u);
     const uint32_t wcol = blockIdx.x * 128u + threadIdx.x;
     if (wcol >= W) return;
     const uint32_t chunk = blockIdx.y, replica = blockIdx.z, n_chunks = gridDim.y;
@@ -128,7 +125,7 @@ __global__ void __launch_bounds__(128) kpz_column_chunk_kernel(const uint32_t* _
         for (int c = 0; c < 32; ++c) {
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                const uint32_t e = mylut[((a[c] >> (8 * q)) & 0xFFu) << 5];
+                const uint32_t e = lut[(a[c] >> (8 * q)) & 0xFFu];
                 const int32_t S0 = (int32_t)(int8_t)(e & 0xFFu), S1 = (int32_t)(int8_t)((e >> 8) & 0xFFu);
                 const int32_t S2 = (int32_t)(e >> 16);
                 const int32_t t = 8 * B[c] + S1;
