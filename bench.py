@@ -282,7 +282,8 @@ def run_ours(args):
         "peak_derived_source": "%d SM x 4 schedulers x 16 ALU lanes/clk x clocks.max.sm (%s MEASURED_PEAKS.json)" % (pk["n_sms"], src),
         "frac_of_derived": upd_rate * alu_ops / alu_peak_derived,
         "measured_peaks": {kk: (v / 1e12 if kk.endswith("ops") or kk == "lds_bytes" else v) for kk, v in pk.items()},
-        "measured_peaks_units": "T lane-ops/s (lop3, shf, imad, imad_wide, smem_xor), TB/s (lds_bytes), attempts/s (attempt_mix), Hz, count",
+        "measured_peaks_units": "T lane-ops/s (lop3, shf, imad, imad_wide, smem_xor), TB/s (lds_bytes), attempts/s (attempt_mix), Hz, count, "
+                                "SM clocks per attempt and warp of one tile's dependent chain at 1 and 2 warps per scheduler (chain_cycles_*)",
         # the shared-memory data pipe is the other co-limit: 5 loads + 1 XOR reduction of 4 bytes per update
         "lsu": {"bound": "shared-memory data pipe", "achieved": upd_rate * ALG_SMEM_BYTES_PER_UPDATE / 1e12,
                 "peak": pk["lds_bytes"] / 1e12, "unit": "TB/s", "frac": upd_rate * ALG_SMEM_BYTES_PER_UPDATE / pk["lds_bytes"],

@@ -228,9 +228,12 @@ int32_t kpz_launch_count(const kpz_ctx* ctx, uint64_t* out);
  *   [6] shared-memory XOR reductions (ATOMS / RED) in lane-operations/s
  *   [7] attempts/s of the bare instruction mix of one p = 1, q = 0 attempt (5 LDS, 2 SHF, 3 LOP3, 1 reduction) issued
  *       without the dependent chain of a real tile -- what the update kernel would reach with perfect latency hiding
- *   [8] number of SMs.
+ *   [8] number of SMs
+ *   [9], [10] SM clocks per attempt and warp of the dependent chain of ONE tile (5 LDS -> 2 SHF -> 3 LOP3 -> XOR
+ *       reduction -> the next attempt's loads) with one and with two warps per scheduler on one SM: the latency that
+ *       only other resident warps can hide.
  * Takes a few tens of milliseconds.  KPZ_EINVAL for a NULL / short array, KPZ_ECUDA without a device. */
-#define KPZ_N_PEAKS 9
+#define KPZ_N_PEAKS 11
 int32_t kpz_measure_peaks(double* out, uint32_t n);
 
 /* Device Philox4x32-10 self-test: evaluates n (counter,key) inputs on the GPU.  HOST arrays: ctr[4n], key[2n],

@@ -92,11 +92,11 @@ def workspace_bytes(L, tile, n_replicas=1):
 
 
 PEAK_NAMES = ("sm_clock_hz", "lop3_lane_ops", "shf_lane_ops", "imad_lane_ops", "imad_wide_lane_ops", "lds_bytes",
-              "smem_xor_lane_ops", "attempt_mix", "n_sms")
+              "smem_xor_lane_ops", "attempt_mix", "n_sms", "chain_cycles_w1", "chain_cycles_w2")
 
 
 def measure_peaks():
-    """kpz_measure_peaks on the current device -> dict of the nine figures (per second, see include/kpz.h)."""
+    """kpz_measure_peaks on the current device -> dict of its figures (see include/kpz.h)."""
     out = np.zeros(len(PEAK_NAMES), dtype=np.float64)
     rc = load_library().kpz_measure_peaks(out.ctypes.data, len(out))
     if rc != KPZ_OK:

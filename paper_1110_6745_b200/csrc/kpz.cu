@@ -844,6 +844,15 @@ int32_t kpz_measure_peaks(double* out, uint32_t n) {
     if (e == cudaSuccess) e = run_peak<kpz::PEAK_LDS>(blocks, iters, sink, ticks, &ms[4]);
     if (e == cudaSuccess) e = run_peak<kpz::PEAK_ATOMS>(blocks, iters, sink, ticks, &ms[5]);
     if (e == cudaSuccess) e = run_peak<kpz::PEAK_MIX>(blocks, iters / 4, sink, ticks, &ms[6]);
+    // the dependent chain of one tile: 1 and 2 warps per scheduler on one SM
+    unsigned long long cticks[2] = {0, 0};
+    for (int v = 0; v < 2 && e == cudaSuccess; ++v) {
+        const uint32_t citers = 50000;
+        kpz::kpz_chain_kernel<<<1, v == 0 ? 128 : 256>>>(citers, 1234u, ticks);
+        e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaMemcpy(&cticks[v], ticks, 8, cudaMemcpyDeviceToHost);
+        out[9 + v] = (double)cticks[v] / citers;
+    }
     cudaFree(sink);
     cudaFree(ticks);
     if (e != cudaSuccess) return KPZ_ECUDA;

@@ -87,4 +87,28 @@ __global__ void __launch_bounds__(256) kpz_peak_kernel(uint32_t iters, uint32_t 
     }
 }
 
+// The dependent chain of one tile: 5 LDS (random row of a private 66-row tile) -> 2 funnel shifts -> 3 LOP3 -> XOR
+// reduction, the next attempt's loads issued after the reduction as in the update kernel (the site sequence does not
+// depend on the tile).  One CTA on one SM; reports clock64 ticks per attempt of warp 0 -- the latency that only other
+// warps can hide.  With w warps per scheduler the per-scheduler cost follows 17 + 48 / w cycles on B200.
+__global__ void __launch_bounds__(512) kpz_chain_kernel(uint32_t iters, uint32_t seed, unsigned long long* __restrict__ ticks) {
+    __shared__ uint32_t sm[32 * 72];
+    for (uint32_t i = threadIdx.x; i < 32 * 72; i += blockDim.x) sm[i] = i * 2654435761u ^ seed;
+    __syncthreads();
+    uint32_t* mine = sm + (threadIdx.x & 31u);
+    uint32_t w = seed + threadIdx.x;
+    const long long t0 = clock64();
+#pragma unroll 4
+    for (uint32_t it = 0; it < iters; ++it) {
+        w = w * 1664525u + 1013904223u;
+        uint32_t* a = mine + 32u * ((w >> 26) + 2u);
+        const uint32_t wo = a[0], wd = a[-32], wu = a[32], wp = a[-64], wn = a[64];
+        const uint32_t wl = __funnelshift_l(wp, wo, 1), wr = __funnelshift_r(wo, wn, 1);
+        const uint32_t t1 = (wo ^ ~wl) | (wo ^ wr), t2 = (wo ^ wu) | (wo ^ ~wd);
+        atomicXor(a, (1u << ((w >> 20) & 31u)) & ~t1 & ~t2);
+    }
+    const long long t1 = clock64();
+    if (threadIdx.x == 0) ticks[0] = (unsigned long long)(t1 - t0);
+}
+
 }  // namespace kpz
