@@ -60,7 +60,13 @@ struct UpdateParams {
     uint32_t tp_incl, tq_incl;     // thr - 1 (MODE 1: both thresholds >= 1, accept iff word <= thr - 1)
     uint32_t L, NT, HN;            // lattice edge, tiles per edge, NT/2
     uint32_t W;                    // L/32: words per bit-line
-    uint32_t tiles_per_colour;     // HN*HN
+    uint32_t tiles_per_colour;     // HN * HNy
+    // A handle may hold one SLAB of the lattice: `rows` consecutive rows starting at global
+    // tile row ty0 (storage row 0 = global row ty0 * T), tile rows ty0 .. ty0 + 2 HNy - 1 of the shifted frame.  The
+    // whole lattice is the case rows = ywrap = L, ty0 = 0, HNy = HN.
+    uint32_t HNy;                  // tile rows of one colour in this launch
+    uint32_t ty0;                  // first global tile row of the stored rows
+    uint32_t ywrap;                // row index at which the stored rows wrap around: L, or 0xFFFFFFFF for a slab (never)
     uint32_t blocked;              // 1: 8x4 lane blocking of tiles (HN % 8 == 0), 0: linear
     uint32_t m;                    // MCS index (number of completed MCS)
     uint32_t slot;                 // 0..3: which entry of the colour order this launch executes
@@ -678,25 +684,28 @@ __global__ void __launch_bounds__(NTHR, (T == 64) ? 3 : (T == 32 ? 8 : 1)) kpz_u
     }
     uint32_t ox, oy, colour;
     global_draw<T>(P, SUB ? P.sub : 0u, replica, ox, oy, colour);
-    const uint32_t tx = DEAD ? i : 2u * i + (colour & 1u), ty = DEAD ? j : 2u * j + (colour >> 1);
-    const uint32_t X0 = ox + tx * T, Y0 = oy + ty * T;        // < L + T
+    const uint32_t tx = DEAD ? i : 2u * i + (colour & 1u), tyl = DEAD ? j : 2u * j + (colour >> 1);
+    const uint32_t ty = tyl + P.ty0;                          // global tile row (tyl: within the stored rows)
+    const uint32_t X0 = ox + tx * T, Y0 = oy + tyl * T;       // < L + T
     const uint32_t tile_id = ty * P.NT + tx;
     uint32_t* planeX = P.lattice + (size_t)replica * 2u * P.plane_words;
     uint32_t* planeY = planeX + P.plane_words;
-    const uint32_t L = P.L, W = P.W;
+    const uint32_t L = P.L, W = P.W, LY = P.ywrap;
     const uint32_t x0 = (X0 >= L) ? X0 - L : X0;   // first own column = bit offset inside a row
-    const uint32_t y0 = (Y0 >= L) ? Y0 - L : Y0;   // first own row
+    const uint32_t y0 = (Y0 >= LY) ? Y0 - LY : Y0; // first own row (storage index)
+    const uint32_t Yg = oy + ty * T;               // ... and as a global row, for the origin test
+    const uint32_t yg0 = (Yg >= L) ? Yg - L : Yg;
 
     uint32_t n_dep = 0, n_rem = 0, n_att = 0;
     int32_t dh00 = 0;
     uint32_t origin_idx = 0xFFFFFFFFu;
     if (active) {
         // ---- a2: stage tile + halo ----
-        if constexpr (G::WIDE) stage_in_wide<T, NTHR>(planeX, planeY, L, W, x0, y0, sm);
-        else stage_in_narrow<T, NTHR>(planeX, planeY, L, W, x0, y0, sm);
-        // does this tile hold global site (0,0)?  its local coordinates: (L - x0) mod L, (L - y0) mod L
+        if constexpr (G::WIDE) stage_in_wide<T, NTHR>(planeX, planeY, LY, W, x0, y0, sm);
+        else stage_in_narrow<T, NTHR>(planeX, planeY, LY, W, x0, y0, sm);
+        // does this tile hold global site (0,0)?  its local coordinates: (L - x0) mod L, (L - yg0) mod L
         const uint32_t lx0 = (x0 == 0u) ? 0u : L - x0;
-        const uint32_t ly0 = (y0 == 0u) ? 0u : L - y0;
+        const uint32_t ly0 = (yg0 == 0u) ? 0u : L - yg0;
         if (lx0 < (uint32_t)T && ly0 < (uint32_t)T) origin_idx = ly0 * T + lx0;
     }
     const bool any_origin = __any_sync(0xFFFFFFFFu, origin_idx != 0xFFFFFFFFu);
@@ -719,8 +728,8 @@ __global__ void __launch_bounds__(NTHR, (T == 64) ? 3 : (T == 32 ? 8 : 1)) kpz_u
         else
             run_tile_steps<T, NTHR, MODE, false, DEAD, SUB>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx, n_steps);
         // ---- a5: write back ----
-        if constexpr (G::WIDE) stage_out_wide<T, NTHR, StageBatch<T>::N, DEAD>(planeX, planeY, L, W, x0, y0, sm);
-        else stage_out_narrow<T, NTHR, DEAD>(planeX, planeY, L, W, x0, y0, sm);
+        if constexpr (G::WIDE) stage_out_wide<T, NTHR, StageBatch<T>::N, DEAD>(planeX, planeY, LY, W, x0, y0, sm);
+        else stage_out_narrow<T, NTHR, DEAD>(planeX, planeY, LY, W, x0, y0, sm);
     }
     // ---- a6: bookkeeping ----
     const uint32_t rep0 = __shfl_sync(0xFFFFFFFFu, replica, 0);
