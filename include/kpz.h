@@ -216,6 +216,49 @@ int32_t kpz_profiles(kpz_ctx* ctx, uint32_t replica, int64_t* col_sums, int64_t*
  * kpz_set_sub_sweeps(K >= 2) removes them. */
 int32_t kpz_power_spectrum(kpz_ctx* ctx, uint32_t replica, double* S, double* Sx, double* Sy);
 
+/* ---- one lattice split into slabs of rows over several handles / GPUs ------------------
+ * For lattices larger than one GPU (L > 2^19), and as the data-parallel form of a single large lattice.  Slab s of
+ * n_slabs owns the L / n_slabs lattice rows from row s * L / n_slabs and the tile rows s * NT / n_slabs .. of the
+ * shifted frame (NT = L / tile; NT must be a multiple of 2 * n_slabs and L / n_slabs a multiple of 32).  Its buffer
+ * stores the owned rows followed by tile + 2 GHOST rows, a copy of the first rows of the next slab (periodically: the
+ * last slab's ghost rows are the first rows of slab 0), in the device layout of a whole lattice with L / n_slabs +
+ * tile + 2 rows per plane.  The tiles of a slab's last tile row reach oy + 1 rows into the ghost rows (oy = the y
+ * origin of the MCS, kpz_global_draw); they are active in the two colour passes whose colour has bit 1 set.  The
+ * DRIVER (paper_1110_6745_b200/slabs.py; any code that can copy device memory between the handles) therefore runs,
+ * for every MCS m and slot = 0..3 with colour = perm[slot]:
+ *     if colour & 2:  copy rows [0, oy + 1) of both planes of slab s+1 into the ghost rows of slab s     (all s)
+ *     kpz_slab_pass(slab s, slot)                                                                     (all s)
+ *     if colour & 2:  copy the ghost rows [0, oy + 1) of slab s back onto rows [0, oy + 1) of slab s+1  (all s)
+ * then kpz_slab_end_mcs on every slab.  The trajectory is the whole-lattice one bit for bit (same tile ids, same
+ * streams; tests/test_gpu_parity.py: test_slabs_*).  Default schedule S4 only; one replica.
+ * Measurement: kpz_slab_measure_local on every slab (column walks of its owned rows; slab 0 also walks row 0 along
+ * x); gather the n_slabs per-column step totals ([n_slabs][L] int32, device) and slab 0's row-0 prefix ([L] int32);
+ * kpz_slab_measure_finish on every slab gives four 64-bit half-accumulators; their sums mod 2^64 over the slabs and the
+ * sum of the slabs' h(0,0) counters go to kpz_slab_finalize.  kpz_init_flat, kpz_counters (per slab: add them up),
+ * kpz_export_packed / kpz_import_packed (the slab's own buffer), kpz_synchronize and kpz_destroy work on slab
+ * handles; the calls that address a whole lattice return KPZ_ESTATE. */
+int32_t kpz_slab_workspace_bytes(uint32_t L, uint32_t tile, uint32_t n_slabs, size_t* lattice_bytes, size_t* scratch_bytes);
+int32_t kpz_create_slab(kpz_ctx** out, uint32_t L, double p, double q, uint32_t tile, uint64_t seed, uint32_t n_slabs,
+                        uint32_t slab);
+/* HOST out-pointers (any may be NULL): rows owned, rows stored (owned + ghost), bytes of one row of one plane (L / 8),
+ * byte offsets INSIDE THE BOUND SCRATCH BUFFER of the row-0 prefix ([L] int32, valid on slab 0 after
+ * kpz_slab_measure_local) and of this slab's per-column step totals ([L] int32). */
+int32_t kpz_slab_info(const kpz_ctx* ctx, uint32_t* rows_own, uint32_t* rows_stored, size_t* row_bytes, size_t* base_offset,
+                      size_t* totals_offset);
+/* Global draw S2 of MCS m evaluated on the host (replica 0): origin (ox, oy) and the colour order perm[4] (HOST out). */
+int32_t kpz_global_draw(const kpz_ctx* ctx, uint64_t m, uint32_t* ox, uint32_t* oy, uint32_t* perm);
+/* Colour pass `slot` (0..3) of the current MCS on this slab's tiles (one launch, asynchronous). */
+int32_t kpz_slab_pass(kpz_ctx* ctx, uint32_t slot);
+/* Advances this slab's MCS clock by one (after the four passes). */
+int32_t kpz_slab_end_mcs(kpz_ctx* ctx);
+int32_t kpz_slab_measure_local(kpz_ctx* ctx);
+/* d_base0: DEVICE [L] int32 row-0 prefix of slab 0; d_totals_all: DEVICE [n_slabs][L] int32 step totals of all slabs;
+ * halves: HOST [4] out.  Synchronises. */
+int32_t kpz_slab_measure_finish(kpz_ctx* ctx, const void* d_base0, const void* d_totals_all, uint64_t* halves);
+/* halves: HOST [4], summed mod 2^64 over the slabs; h00: sum of the slabs' h(0,0) counters.  Outputs as kpz_measure
+ * (HOST, any may be NULL); KPZ_EOVERFLOW as kpz_measure. */
+int32_t kpz_slab_finalize(uint32_t L, const uint64_t* halves, int64_t h00, int64_t* sum_h, int64_t* sum_h2, double* W2);
+
 /* Number of kernels this handle has launched since creation (for bench.py "gpu_launches"). */
 int32_t kpz_launch_count(const kpz_ctx* ctx, uint64_t* out);
 

@@ -23,6 +23,8 @@ exported_symbols = [
     "kpz_state_hash", "kpz_counters", "kpz_export_packed", "kpz_import_packed", "kpz_step_host", "kpz_pipeline_host",
     "kpz_launch_count", "kpz_philox_selftest", "kpz_profiles", "kpz_power_spectrum", "kpz_set_schedule", "kpz_set_sub_sweeps", "kpz_run_sampled", "kpz_set_poisson",
     "kpz_set_path", "kpz_measure_peaks",
+    "kpz_slab_workspace_bytes", "kpz_create_slab", "kpz_slab_info", "kpz_global_draw", "kpz_slab_pass", "kpz_slab_end_mcs",
+    "kpz_slab_measure_local", "kpz_slab_measure_finish", "kpz_slab_finalize",
 ]
 
 
@@ -72,6 +74,15 @@ def load_library() -> ctypes.CDLL:
         "kpz_launch_count": [vp, vp],
         "kpz_philox_selftest": [vp, vp, vp, u32],
         "kpz_measure_peaks": [vp, u32],
+        "kpz_slab_workspace_bytes": [u32, u32, u32, vp, vp],
+        "kpz_create_slab": [vp, u32, dbl, dbl, u32, u64, u32, u32],
+        "kpz_slab_info": [vp, vp, vp, vp, vp, vp],
+        "kpz_global_draw": [vp, u64, vp, vp, vp],
+        "kpz_slab_pass": [vp, u32],
+        "kpz_slab_end_mcs": [vp],
+        "kpz_slab_measure_local": [vp],
+        "kpz_slab_measure_finish": [vp, vp, vp, vp],
+        "kpz_slab_finalize": [u32, vp, i64, vp, vp, vp],
     }
     for name, args in sig.items():
         fn = getattr(L, name)

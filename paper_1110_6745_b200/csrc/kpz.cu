@@ -98,9 +98,16 @@ void fill_update_params(const kpz_ctx* c, kpz::UpdateParams& P, uint32_t m, uint
     P.NT = c->L / c->T;
     P.HN = (c->schedule == KPZ_SCHEDULE_DEAD_BORDER) ? P.NT : P.NT / 2;   // tiles per edge in one launch
     P.W = c->L / 32;
-    P.tiles_per_colour = P.HN * P.HN;
+    // whole lattice: all L rows stored, tile rows from 0, rows wrap at L.  A slab handle (kpz_create_slab) stores
+    // rows_own + ghost rows from global tile row slab * NT / n_slabs on, never wraps, and runs NT / n_slabs tile rows.
+    const bool slab = c->n_slabs > 0;
+    P.HNy = slab ? P.NT / c->n_slabs / 2 : P.HN;
+    P.ty0 = slab ? c->slab * (P.NT / c->n_slabs) : 0u;
+    P.ywrap = slab ? 0xFFFFFFFFu : c->L;
+    if (slab) P.plane_words = (uint64_t)c->rows * (c->L / 32);
+    P.tiles_per_colour = P.HN * P.HNy;
     P.total_items = (uint64_t)c->R * P.tiles_per_colour;
-    P.blocked = (P.HN % 8 == 0) ? 1u : 0u;
+    P.blocked = (P.HN % 8 == 0 && P.HNy % 4 == 0) ? 1u : 0u;
     P.thr_p = accept_threshold(c->p);
     P.thr_q = accept_threshold(c->q);
     P.tp_incl = (uint32_t)(P.thr_p - 1);
@@ -182,6 +189,44 @@ int32_t require_bound(kpz_ctx* c) {
     return KPZ_OK;
 }
 
+// entry points that address the lattice as a whole (windows, hash, profiles, kpz_run, kpz_measure ...)
+int32_t require_whole(kpz_ctx* c) {
+    if (c->n_slabs > 0) return kpz_fail(c, KPZ_ESTATE, "not available on a slab handle (use the kpz_slab_* calls)");
+    return KPZ_OK;
+}
+
+// host evaluation of the global draw S2 (the kernels evaluate the same draw in-kernel; the slab driver needs the
+// origin and the colour order to know which rows to exchange)
+void host_philox4x32_10(uint32_t c[4], uint32_t k0, uint32_t k1) {
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c[0], p1 = (uint64_t)0xCD9E8D57u * c[2];
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c[1] ^ k0, n2 = (uint32_t)(p0 >> 32) ^ c[3] ^ k1;
+        c[1] = (uint32_t)p1; c[3] = (uint32_t)p0; c[0] = n0; c[2] = n2;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+}
+
+void host_global_draw(const kpz_ctx* c, uint32_t m, uint32_t sub, uint32_t replica, uint32_t* ox, uint32_t* oy, uint32_t perm[4]) {
+    uint32_t G[4] = {sub, 0xFFFFFFFFu, m, replica};
+    host_philox4x32_10(G, (uint32_t)(c->seed & 0xFFFFFFFFull), (uint32_t)(c->seed >> 32));
+    const uint32_t g = 4, T = c->T;
+    *ox = g * (uint32_t)(((uint64_t)G[0] * (T / g)) >> 32);
+    *oy = g * (uint32_t)(((uint64_t)G[1] * (T / g)) >> 32);
+    const uint32_t pidx = (uint32_t)(((uint64_t)G[2] * 24u) >> 32);
+    const uint32_t d[3] = {pidx / 6u, (pidx % 6u) / 2u, pidx % 2u};
+    uint32_t pool[4] = {0, 1, 2, 3};
+    int n = 4;
+    for (int k = 0; k < 3; ++k) {
+        perm[k] = pool[d[k]];
+        for (int j = (int)d[k]; j < n - 1; ++j) pool[j] = pool[j + 1];
+        --n;
+    }
+    perm[3] = pool[0];
+}
+
+// sum h, sum h^2, W^2 of one lattice from the sums relative to h(0,0) (R16: 128-bit integers, one conversion, one division)
+bool finalize_sums(uint32_t L, i128 S1, i128 S2, long long h00, int64_t* sum_h, int64_t* sum_h2, double* W2);
+
 // sums for all replicas -> host vectors (relative to h(0,0)) + h00
 int32_t measure_relative(kpz_ctx* c, std::vector<i128>& S1, std::vector<i128>& S2, std::vector<long long>& h00,
                          bool want_colsum = false, uint32_t colsum_replica = 0) {
@@ -200,12 +245,12 @@ int32_t measure_relative(kpz_ctx* c, std::vector<i128>& S1, std::vector<i128>& S
     KPZ_CUDA(c, cudaGetLastError());
     dim3 g1((W + 127) / 128, c->sl.n_chunks, R);
     kpz::kpz_column_chunk_kernel<<<g1, 128, 0, c->stream>>>(c->d_lattice, plane_words, L, W, c->sl.rows_per_chunk, cS0,
-                                                         cS1, cS2);
+                                                         cS1, cS2, L, 1u);
     KPZ_CUDA(c, cudaGetLastError());
     dim3 g2((L + 255) / 256, R);
     kpz::kpz_combine_kernel<<<g2, 256, 0, c->stream>>>(base, cS0, cS1, cS2, L, c->sl.n_chunks, c->sl.rows_per_chunk, msum,
                                                     want_colsum ? reinterpret_cast<long long*>(sc + c->sl.colsum) : nullptr,
-                                                    colsum_replica);
+                                                    colsum_replica, L);
     KPZ_CUDA(c, cudaGetLastError());
     c->launches += 3;
     std::vector<unsigned long long> hm((size_t)R * 4), hs((size_t)R * 4);
@@ -222,6 +267,22 @@ int32_t measure_relative(kpz_ctx* c, std::vector<i128>& S1, std::vector<i128>& S
 }
 
 bool fits_i64(i128 v) { return v >= (i128)INT64_MIN && v <= (i128)INT64_MAX; }
+
+// returns true if a requested int64 output overflowed (it is then written as 0)
+bool finalize_sums(uint32_t L, i128 S1, i128 S2, long long h00, int64_t* sum_h, int64_t* sum_h2, double* W2) {
+    const i128 N = (i128)L * L;
+    const double Nd = (double)((uint64_t)L * L);
+    const i128 h0 = h00;
+    const i128 sh = S1 + N * h0;                          // sum h
+    const i128 sh2 = S2 + 2 * h0 * S1 + N * h0 * h0;      // sum h^2
+    // N*sum_h2 - sum_h^2 is invariant under the shift by h0: evaluate it on the small relative sums
+    const i128 num = N * S2 - S1 * S1;
+    bool overflow = false;
+    if (W2) *W2 = (double)num / (Nd * Nd);
+    if (sum_h) { if (fits_i64(sh)) *sum_h = (int64_t)sh; else { *sum_h = 0; overflow = true; } }
+    if (sum_h2) { if (fits_i64(sh2)) *sum_h2 = (int64_t)sh2; else { *sum_h2 = 0; overflow = true; } }
+    return overflow;
+}
 
 }  // namespace
 
@@ -279,6 +340,7 @@ int32_t kpz_create_batch(kpz_ctx** out, uint32_t L, double p, double q, uint32_t
     c->mcs = 0; c->launches = 0; c->schedule = KPZ_SCHEDULE_COLOURS; c->sub_sweeps = 1;
     c->poisson = false; c->pn = 0; c->pk_min = 0; c->attempts_base = 0; c->path = KPZ_PATH_AUTO;
     c->d_lattice = nullptr; c->d_scratch = nullptr; c->stream = nullptr; c->bound = false; c->device = -1; c->s_in = nullptr; c->s_out = nullptr;
+    c->n_slabs = 0; c->slab = 0; c->rows_own = L; c->rows = L;
     c->sl = scratch_layout(L, n_replicas);
     c->lattice_bytes = (size_t)n_replicas * ((size_t)L * L / 4);
     c->err[0] = 0;
@@ -318,7 +380,7 @@ int32_t kpz_init_flat(kpz_ctx* c) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
-    const uint64_t n_words = (uint64_t)c->R * ((uint64_t)c->L * c->L / 16);
+    const uint64_t n_words = c->lattice_bytes / 4;      // both planes of every replica (of the stored rows of a slab)
     kpz::kpz_fill_flat_kernel<<<grid_for(n_words, 256, 148 * 32), 256, 0, c->stream>>>(c->d_lattice, n_words, c->L / 32);
     KPZ_CUDA(c, cudaGetLastError());
     c->launches++;
@@ -332,6 +394,7 @@ int32_t kpz_run(kpz_ctx* c, uint64_t mcs) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
+    if ((rc = require_whole(c)) != KPZ_OK) return rc;
     if (c->mcs + mcs > 0xFFFFFFFFull) return kpz_fail(c, KPZ_EINVAL, "MCS clock would exceed 2^32-1");
     if (mcs == 0) return KPZ_OK;
     ResidentPlan pl{};
@@ -415,6 +478,7 @@ int32_t kpz_set_poisson(kpz_ctx* c, int32_t on) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
+    if ((rc = require_whole(c)) != KPZ_OK) return rc;
     c->poisson = on != 0;
     return c->poisson ? upload_poisson_table(c) : KPZ_OK;
 }
@@ -423,23 +487,15 @@ int32_t kpz_measure(kpz_ctx* c, int64_t* sum_h, int64_t* sum_h2, double* W2) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
+    if ((rc = require_whole(c)) != KPZ_OK) return rc;
     std::vector<i128> S1, S2;
     std::vector<long long> h00;
     rc = measure_relative(c, S1, S2, h00);
     if (rc != KPZ_OK) return rc;
-    const i128 N = (i128)c->L * c->L;
-    const double Nd = (double)((uint64_t)c->L * c->L);
     bool overflow = false;
-    for (uint32_t r = 0; r < c->R; ++r) {
-        const i128 h0 = h00[r];
-        const i128 sh = S1[r] + N * h0;                          // sum h
-        const i128 sh2 = S2[r] + 2 * h0 * S1[r] + N * h0 * h0;   // sum h^2
-        // N*sum_h2 - sum_h^2 is invariant under the shift by h0: evaluate it on the small relative sums
-        const i128 num = N * S2[r] - S1[r] * S1[r];
-        if (W2) W2[r] = (double)num / (Nd * Nd);
-        if (sum_h) { if (fits_i64(sh)) sum_h[r] = (int64_t)sh; else { sum_h[r] = 0; overflow = true; } }
-        if (sum_h2) { if (fits_i64(sh2)) sum_h2[r] = (int64_t)sh2; else { sum_h2[r] = 0; overflow = true; } }
-    }
+    for (uint32_t r = 0; r < c->R; ++r)
+        overflow |= finalize_sums(c->L, S1[r], S2[r], h00[r], sum_h ? sum_h + r : nullptr, sum_h2 ? sum_h2 + r : nullptr,
+                                  W2 ? W2 + r : nullptr);
     if (overflow) return kpz_fail(c, KPZ_EOVERFLOW, "a sum does not fit int64");
     return KPZ_OK;
 }
@@ -492,6 +548,7 @@ int32_t kpz_get_window(kpz_ctx* c, uint32_t replica, uint32_t x0, uint32_t y0, u
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
+    if ((rc = require_whole(c)) != KPZ_OK) return rc;
     if (replica >= c->R || !sx || !sy || w == 0 || h == 0 || w > c->L || h > c->L) return kpz_fail(c, KPZ_EINVAL, "bad window");
     const size_t n = (size_t)w * h;
     int8_t* d = nullptr;
@@ -517,6 +574,7 @@ int32_t kpz_set_slopes(kpz_ctx* c, uint32_t replica, const int8_t* sx, const int
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
+    if ((rc = require_whole(c)) != KPZ_OK) return rc;
     if (replica >= c->R || !sx || !sy) return kpz_fail(c, KPZ_EINVAL, "bad argument");
     const size_t n = (size_t)c->L * c->L;
     int8_t* d = nullptr;
@@ -554,6 +612,7 @@ int32_t kpz_state_hash(kpz_ctx* c, uint32_t replica, uint64_t* out) {
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
+    if ((rc = require_whole(c)) != KPZ_OK) return rc;
     if (replica >= c->R || !out) return kpz_fail(c, KPZ_EINVAL, "bad argument");
     unsigned long long* acc = reinterpret_cast<unsigned long long*>(c->d_scratch + c->sl.misc);
     const uint64_t plane_words = (uint64_t)c->L * c->L / 32;
@@ -675,6 +734,7 @@ int32_t kpz_pipeline_host(kpz_ctx* c, void* device_lattice2, size_t device_latti
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
+    if ((rc = require_whole(c)) != KPZ_OK) return rc;
     if (!device_lattice2 || device_lattice2_bytes < c->lattice_bytes || ((uintptr_t)device_lattice2 & 15u))
         return kpz_fail(c, KPZ_EINVAL, "second device lattice missing, too small or not 16-byte aligned");
     if (n_lanes == 0 || n_rounds == 0 || !host_lattices || !mcs_start || bytes < c->lattice_bytes)
@@ -785,6 +845,7 @@ int32_t kpz_profiles(kpz_ctx* c, uint32_t replica, int64_t* col_sums, int64_t* r
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
+    if ((rc = require_whole(c)) != KPZ_OK) return rc;
     if (replica >= c->R) return kpz_fail(c, KPZ_EINVAL, "replica out of range");
     long long h00 = 0;
     rc = run_profiles(c, replica, false, &h00);
@@ -804,6 +865,7 @@ int32_t kpz_power_spectrum(kpz_ctx* c, uint32_t replica, double* S, double* Sx, 
     int32_t rc = require_bound(c);
     if (rc != KPZ_OK) return rc;
     DeviceGuard dg__(c->device);
+    if ((rc = require_whole(c)) != KPZ_OK) return rc;
     if (replica >= c->R) return kpz_fail(c, KPZ_EINVAL, "replica out of range");
     long long h00 = 0;
     rc = run_profiles(c, replica, true, &h00);
@@ -814,6 +876,140 @@ int32_t kpz_power_spectrum(kpz_ctx* c, uint32_t replica, double* S, double* Sx, 
     if (Sy) KPZ_CUDA(c, cudaMemcpyAsync(Sy, c->d_scratch + c->sl.sdir + n * 8, n * 8, cudaMemcpyDeviceToHost, c->stream));
     KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
     return KPZ_OK;
+}
+
+
+// ---- one lattice split into slabs of rows over several handles / GPUs ---------------------
+
+int32_t kpz_slab_workspace_bytes(uint32_t L, uint32_t tile, uint32_t n_slabs, size_t* lattice_bytes, size_t* scratch_bytes) {
+    int32_t rc = validate(L, 0.0, 0.0, tile, 1);
+    if (rc != KPZ_OK) return rc;
+    if (n_slabs == 0 || (L / tile) % (2 * n_slabs) != 0 || (L / n_slabs) % 32 != 0) return KPZ_EINVAL;
+    const size_t rows = (size_t)L / n_slabs + tile + 2;
+    if (lattice_bytes) *lattice_bytes = 2 * rows * (L / 8);
+    if (scratch_bytes) *scratch_bytes = scratch_layout(L, 1).total;
+    return KPZ_OK;
+}
+
+int32_t kpz_create_slab(kpz_ctx** out, uint32_t L, double p, double q, uint32_t tile, uint64_t seed, uint32_t n_slabs,
+                        uint32_t slab) {
+    if (!out) return KPZ_EINVAL;
+    *out = nullptr;
+    size_t lat = 0;
+    int32_t rc = kpz_slab_workspace_bytes(L, tile, n_slabs, &lat, nullptr);
+    if (rc != KPZ_OK || slab >= n_slabs) return KPZ_EINVAL;
+    rc = kpz_create_batch(out, L, p, q, tile, seed, 1);
+    if (rc != KPZ_OK) return rc;
+    kpz_ctx* c = *out;
+    c->n_slabs = n_slabs;
+    c->slab = slab;
+    c->rows_own = L / n_slabs;
+    c->rows = c->rows_own + tile + 2;
+    c->lattice_bytes = lat;
+    return KPZ_OK;
+}
+
+int32_t kpz_slab_info(const kpz_ctx* c, uint32_t* rows_own, uint32_t* rows_stored, size_t* row_bytes, size_t* base_offset,
+                      size_t* totals_offset) {
+    if (!c || c->n_slabs == 0) return KPZ_EINVAL;
+    if (rows_own) *rows_own = c->rows_own;
+    if (rows_stored) *rows_stored = c->rows;
+    if (row_bytes) *row_bytes = c->L / 8;
+    if (base_offset) *base_offset = c->sl.base;
+    if (totals_offset) *totals_offset = c->sl.rowinc;
+    return KPZ_OK;
+}
+
+int32_t kpz_global_draw(const kpz_ctx* c, uint64_t m, uint32_t* ox, uint32_t* oy, uint32_t* perm) {
+    if (!c || !ox || !oy || !perm || m > 0xFFFFFFFFull) return KPZ_EINVAL;
+    host_global_draw(c, (uint32_t)m, 0u, 0u, ox, oy, perm);
+    return KPZ_OK;
+}
+
+int32_t kpz_slab_pass(kpz_ctx* c, uint32_t slot) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
+    if (c->n_slabs == 0) return kpz_fail(c, KPZ_ESTATE, "not a slab handle");
+    if (slot > 3 || c->schedule != KPZ_SCHEDULE_COLOURS || c->sub_sweeps != 1 || c->poisson)
+        return kpz_fail(c, KPZ_EINVAL, "slabs run the default schedule, colour passes 0..3");
+    if (c->mcs >= 0xFFFFFFFFull) return kpz_fail(c, KPZ_EINVAL, "MCS clock would exceed 2^32-1");
+    return launch_update(c, (uint32_t)c->mcs, slot, 0u);
+}
+
+int32_t kpz_slab_end_mcs(kpz_ctx* c) {
+    if (!c || c->n_slabs == 0) return KPZ_EINVAL;
+    if (c->mcs >= 0xFFFFFFFFull) return kpz_fail(c, KPZ_EINVAL, "MCS clock would exceed 2^32-1");
+    c->mcs++;
+    c->attempts_base += (uint64_t)c->L * c->rows_own;
+    return KPZ_OK;
+}
+
+int32_t kpz_slab_measure_local(kpz_ctx* c) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
+    if (c->n_slabs == 0) return kpz_fail(c, KPZ_ESTATE, "not a slab handle");
+    const uint32_t L = c->L, W = L / 32;
+    const uint64_t plane_words = (uint64_t)c->rows * W;
+    unsigned char* sc = c->d_scratch;
+    int32_t* base = reinterpret_cast<int32_t*>(sc + c->sl.base);
+    int32_t* cS0 = reinterpret_cast<int32_t*>(sc + c->sl.cS0);
+    int32_t* cS1 = reinterpret_cast<int32_t*>(sc + c->sl.cS1);
+    int32_t* cS2 = reinterpret_cast<int32_t*>(sc + c->sl.cS2);
+    if (c->slab == 0) {       // the walk along x on lattice row 0 (eq. 3) lives on slab 0
+        int nthr = 1024;
+        while (nthr > 32 && (uint32_t)nthr > L) nthr >>= 1;
+        kpz::kpz_row0_prefix_kernel<<<1, nthr, 0, c->stream>>>(c->d_lattice, plane_words, L, W, base);
+        KPZ_CUDA(c, cudaGetLastError());
+        c->launches++;
+    }
+    dim3 g1((W + 127) / 128, c->sl.n_chunks, 1);
+    kpz::kpz_column_chunk_kernel<<<g1, 128, 0, c->stream>>>(c->d_lattice, plane_words, L, W, c->sl.rows_per_chunk, cS0, cS1, cS2,
+                                                         c->rows_own, c->slab == 0 ? 1u : 0u);
+    KPZ_CUDA(c, cudaGetLastError());
+    kpz::kpz_slab_totals_kernel<<<(L + 255) / 256, 256, 0, c->stream>>>(cS0, L, c->sl.n_chunks, c->sl.rows_per_chunk, c->rows_own,
+                                                                    reinterpret_cast<int32_t*>(sc + c->sl.rowinc));
+    KPZ_CUDA(c, cudaGetLastError());
+    c->launches += 2;
+    return KPZ_OK;
+}
+
+int32_t kpz_slab_measure_finish(kpz_ctx* c, const void* d_base0, const void* d_totals_all, uint64_t* halves) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
+    if (c->n_slabs == 0) return kpz_fail(c, KPZ_ESTATE, "not a slab handle");
+    if (!d_base0 || !d_totals_all || !halves) return kpz_fail(c, KPZ_EINVAL, "NULL argument");
+    const uint32_t L = c->L;
+    unsigned char* sc = c->d_scratch;
+    unsigned long long* msum = reinterpret_cast<unsigned long long*>(sc + c->sl.msum);
+    KPZ_CUDA(c, cudaMemsetAsync(msum, 0, 32, c->stream));
+    // the entry height of this slab's columns; prof (unused on slab handles) holds it so that base0 may alias `base`
+    int32_t* mybase = reinterpret_cast<int32_t*>(sc + c->sl.prof);
+    kpz::kpz_slab_base_kernel<<<(L + 255) / 256, 256, 0, c->stream>>>(static_cast<const int32_t*>(d_base0),
+                                                                  static_cast<const int32_t*>(d_totals_all), L, c->slab, mybase);
+    KPZ_CUDA(c, cudaGetLastError());
+    dim3 g2((L + 255) / 256, 1);
+    kpz::kpz_combine_kernel<<<g2, 256, 0, c->stream>>>(mybase, reinterpret_cast<int32_t*>(sc + c->sl.cS0),
+                                                    reinterpret_cast<int32_t*>(sc + c->sl.cS1),
+                                                    reinterpret_cast<int32_t*>(sc + c->sl.cS2), L, c->sl.n_chunks,
+                                                    c->sl.rows_per_chunk, msum, nullptr, 0u, c->rows_own);
+    KPZ_CUDA(c, cudaGetLastError());
+    c->launches += 2;
+    unsigned long long hm[4];
+    KPZ_CUDA(c, cudaMemcpyAsync(hm, msum, 32, cudaMemcpyDeviceToHost, c->stream));
+    KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int k = 0; k < 4; ++k) halves[k] = hm[k];
+    return KPZ_OK;
+}
+
+int32_t kpz_slab_finalize(uint32_t L, const uint64_t* halves, int64_t h00, int64_t* sum_h, int64_t* sum_h2, double* W2) {
+    if (!halves || L == 0) return KPZ_EINVAL;
+    // halves: {lo, hi} 32-bit-half accumulators of sum (h - h00) and of sum (h - h00)^2, summed over the slabs
+    const i128 S1 = (i128)(long long)halves[1] * ((i128)1 << 32) + (i128)halves[0];
+    const i128 S2 = (i128)(long long)halves[3] * ((i128)1 << 32) + (i128)halves[2];
+    return finalize_sums(L, S1, S2, (long long)h00, sum_h, sum_h2, W2) ? KPZ_EOVERFLOW : KPZ_OK;
 }
 
 int32_t kpz_launch_count(const kpz_ctx* c, uint64_t* out) {

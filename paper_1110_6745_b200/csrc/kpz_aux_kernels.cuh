@@ -89,7 +89,10 @@ __device__ __forceinline__ void transpose32x32(uint32_t (&a)[32]) {
 __global__ void __launch_bounds__(128) kpz_column_chunk_kernel(const uint32_t* __restrict__ lattice,
                                                                uint64_t plane_words, uint32_t L, uint32_t W,
                                                                uint32_t rows_per_chunk, int32_t* __restrict__ cS0,
-                                                               int32_t* __restrict__ cS1, int32_t* __restrict__ cS2) {
+                                                               int32_t* __restrict__ cS1, int32_t* __restrict__ cS2,
+                                                               uint32_t n_rows, uint32_t row0_is_lattice_row0) {
+    // n_rows stored rows are walked (L for a whole lattice, the owned rows of a slab); L is the number of columns.
+    // row0_is_lattice_row0 = 0 for a slab that does not start at lattice row 0: its first row is an ordinary step.
     // One 256-entry copy for the whole CTA.  (A copy per bank, lut[32 * byte + lane], removes the 1.6e8 bank
     // conflicts of a measurement at L = 2^17 but costs an index shift and 32 KB per CTA: 1.76 ms against 1.54 ms,
     // the kernel is bound by the ALU pipe at 70 %, not by the table -- measured in round 2 and dropped.)
@@ -109,7 +112,7 @@ __global__ void __launch_bounds__(128) kpz_column_chunk_kernel(const uint32_t* _
     const uint32_t chunk = blockIdx.y, replica = blockIdx.z, n_chunks = gridDim.y;
     const uint32_t* planeY = lattice + (size_t)replica * 2u * plane_words + plane_words;
     const uint32_t y_begin = chunk * rows_per_chunk;
-    const uint32_t y_end = min(L, y_begin + rows_per_chunk);
+    const uint32_t y_end = min(n_rows, y_begin + rows_per_chunk);
     int32_t B[32], s1[32], s2[32];
 #pragma unroll
     for (int c = 0; c < 32; ++c) { B[c] = 0; s1[c] = 0; s2[c] = 0; }
@@ -139,7 +142,7 @@ __global__ void __launch_bounds__(128) kpz_column_chunk_kernel(const uint32_t* _
     const size_t o = ((size_t)replica * n_chunks + chunk) * L + (size_t)wcol * 32u;
 #pragma unroll
     for (int c = 0; c < 32; ++c) {
-        if (chunk == 0u) {
+        if (chunk == 0u && row0_is_lattice_row0) {
             const int32_t s0 = ((first_row >> c) & 1u) ? 1 : -1;
             s2[c] += -2 * s0 * s1[c] + n;
             s1[c] -= n * s0;
@@ -158,7 +161,8 @@ __global__ void __launch_bounds__(256) kpz_combine_kernel(const int32_t* __restr
                                                           const int32_t* __restrict__ cS2, uint32_t L,
                                                           uint32_t n_chunks, uint32_t rows_per_chunk,
                                                           unsigned long long* __restrict__ msum,
-                                                          long long* __restrict__ colsum, uint32_t colsum_replica) {
+                                                          long long* __restrict__ colsum, uint32_t colsum_replica,
+                                                          uint32_t n_rows) {
     const uint32_t replica = blockIdx.y;
     const uint32_t x = blockIdx.x * 256u + threadIdx.x;
     long long a1 = 0, a2 = 0;
@@ -166,8 +170,8 @@ __global__ void __launch_bounds__(256) kpz_combine_kernel(const int32_t* __restr
         long long B = base[(size_t)replica * L + x];
         for (uint32_t c = 0; c < n_chunks; ++c) {
             const uint32_t y_begin = c * rows_per_chunk;
-            if (y_begin >= L) break;
-            const long long n = (long long)(min(L, y_begin + rows_per_chunk) - y_begin);
+            if (y_begin >= n_rows) break;
+            const long long n = (long long)(min(n_rows, y_begin + rows_per_chunk) - y_begin);
             const size_t o = ((size_t)replica * n_chunks + c) * L + x;
             const long long S1 = cS1[o], S2 = cS2[o];
             a1 += n * B + S1;
@@ -410,6 +414,29 @@ __global__ void kpz_philox_selftest_kernel(const uint32_t* ctr, const uint32_t* 
     PhiloxKey k{key[2 * t], key[2 * t + 1]};
     const uint4 r = philox4x32_10(ctr[4 * t], ctr[4 * t + 1], ctr[4 * t + 2], ctr[4 * t + 3], k);
     out[4 * t] = r.x; out[4 * t + 1] = r.y; out[4 * t + 2] = r.z; out[4 * t + 3] = r.w;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Slab helpers: per-column step total of a slab's owned rows, and the entry height of a slab
+// from the row-0 prefix and the totals of the slabs below it.
+// ------------------------------------------------------------------------------------------------------------
+__global__ void kpz_slab_totals_kernel(const int32_t* __restrict__ cS0, uint32_t L, uint32_t n_chunks, uint32_t rows_per_chunk,
+                                       uint32_t n_rows, int32_t* __restrict__ tot) {
+    const uint32_t x = blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= L) return;
+    int32_t t = 0;
+    for (uint32_t c = 0; c < n_chunks && c * rows_per_chunk < n_rows; ++c) t += cS0[(size_t)c * L + x];
+    tot[x] = t;
+}
+
+// base[x] = base0[x] + sum_{r' < slab} tot_all[r'][x]
+__global__ void kpz_slab_base_kernel(const int32_t* __restrict__ base0, const int32_t* __restrict__ tot_all, uint32_t L,
+                                     uint32_t slab, int32_t* __restrict__ base) {
+    const uint32_t x = blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= L) return;
+    int32_t b = base0[x];
+    for (uint32_t r = 0; r < slab; ++r) b += tot_all[(size_t)r * L + x];
+    base[x] = b;
 }
 
 }  // namespace kpz

@@ -51,6 +51,8 @@ struct kpz_ctx {
     bool bound;
     ScratchLayout sl;
     size_t lattice_bytes;
+    uint32_t n_slabs, slab;  // > 0: this handle holds slab `slab` of n_slabs of one lattice (kpz_create_slab); 0: a whole lattice
+    uint32_t rows_own, rows; // slab: rows of the lattice this slab owns, rows stored (owned + ghost rows of the next slab)
     int device;              // ordinal of the device that holds the bound buffers (-1 before kpz_bind)
     cudaStream_t s_in, s_out;     // copy streams of kpz_pipeline_host, created on first use, kept for the handle's life
     std::vector<cudaEvent_t> events;   // its event pool (grown on demand, destroyed with the handle)

@@ -879,3 +879,62 @@ def test_pipeline_host_rejects_bad_arguments(pkg):
     o = Oracle(64, 1.0, 0.0, 16, 1)
     o.init_flat(); o.run(1)
     assert k.state_hash() == o.state_hash()
+
+
+@pytest.mark.parametrize("L,T,p,q,seed,N,n", [
+    (256, 16, 1.0, 0.0, 81, 1, 4),           # one slab: the ghost rows wrap onto the slab's own first rows
+    (256, 16, 0.75, 0.25, 82, 2, 5),
+    (512, 16, 1.0, 0.0, 83, 4, 4),
+    (512, 32, 0.6, 0.1, 84, 2, 4),
+    (1024, 64, 1.0, 0.0, 85, 2, 3),
+    (2048, 64, 0.75, 0.25, 86, 4, 3),        # blocked lane mapping inside a slab (HN = 16, 4 tile rows per colour)
+    (1024, 64, 1.0, 0.0, 87, 8, 3),          # one tile row of each parity per slab
+])
+def test_slabs_match_whole_lattice_and_oracle(pkg, L, T, p, q, seed, N, n):
+    """One lattice as N slabs of rows (kpz_create_slab / kpz_slab_pass, paper_1110_6745_b200/slabs.py; all slabs on
+    this GPU, run one after the other): packed state, sums, W^2 and counters after every MCS equal the oracle's and
+    the single-handle lattice's, bit for bit."""
+    import torch
+    from paper_1110_6745_b200.slabs import SlabLattice
+    sl = SlabLattice(L, p, q, T, seed, N)
+    sl.init_flat()
+    k = pkg.KPZ(L, p, q, T, seed)
+    k.set_path("tiled")
+    k.init_flat()
+    o = Oracle(L, p, q, T, seed, threads=NTHREADS)
+    o.init_flat()
+    host = torch.empty(k.lattice_bytes, dtype=torch.uint8).pin_memory()
+    assert sl.measure() == (L * L // 2, L * L // 2, 0.25)
+    for t in range(n):
+        sl.run(1); k.run(1); o.run(1)
+        s1, s2, w2 = k.measure()
+        assert sl.measure() == (int(s1[0]), int(s2[0]), float(w2[0])) == o.measure()
+        k.export_packed(host)
+        assert torch.equal(sl.packed_rows().reshape(-1), host), t
+        assert sl.counters() == k.counters() == o.counters()
+    sl.run(2); o.run(2)                                    # several MCS per call
+    assert sl.measure() == o.measure()
+    sl.close()
+
+
+def test_slab_handles_validate_and_refuse_whole_lattice_calls(pkg):
+    import ctypes
+    from paper_1110_6745_b200.slabs import SlabHandle
+    lib = pkg.load_library()
+    a, b = ctypes.c_size_t(), ctypes.c_size_t()
+    assert lib.kpz_slab_workspace_bytes(256, 16, 3, ctypes.addressof(a), ctypes.addressof(b)) == pkg.KPZ_EINVAL   # NT % (2 N)
+    assert lib.kpz_slab_workspace_bytes(256, 16, 16, ctypes.addressof(a), ctypes.addressof(b)) == pkg.KPZ_EINVAL
+    assert lib.kpz_slab_workspace_bytes(256, 16, 2, ctypes.addressof(a), ctypes.addressof(b)) == pkg.KPZ_OK
+    assert a.value == 2 * (128 + 16 + 2) * 32
+    h = SlabHandle(256, 1.0, 0.0, 16, 1, 2, 1)
+    h.init_flat()
+    out = ctypes.c_uint64()
+    assert lib.kpz_state_hash(h._h, 0, ctypes.addressof(out)) == pkg.KPZ_ESTATE
+    assert lib.kpz_run(h._h, 1) == pkg.KPZ_ESTATE
+    assert lib.kpz_slab_pass(h._h, 4) == pkg.KPZ_EINVAL
+    k = pkg.KPZ(256, 1.0, 0.0, 16, 1)
+    assert lib.kpz_slab_pass(k._h, 0) == pkg.KPZ_ESTATE
+    o = Oracle(256, 1.0, 0.0, 16, 1)
+    for m in (0, 1, 17, 2**32 - 2):
+        assert tuple(h.global_draw(m)) == tuple(o.global_draw(m))      # host evaluation of S2 = the oracle's
+    h.close()
