@@ -341,6 +341,66 @@ def run_ours(args):
     print(json.dumps(out))
 
 
+def run_slabs(args):
+    """--slabs: the config's ONE lattice as N slabs of rows, rank r holding slab r (paper_1110_6745_b200/slabs.py:
+    ghost rows point to point between neighbouring ranks twice per MCS, the measurement through one all_gather, one
+    broadcast and one all_reduce).  Strong scaling: the total work is fixed as N grows."""
+    import torch
+    import torch.distributed as dist
+    from paper_1110_6745_b200 import shard
+    from paper_1110_6745_b200.slabs import DistSlab, SlabHandle
+    rank, world, local = shard.rank_world()
+    if world != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%d" % (args.gpus, world))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    else:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29531")
+        dist.init_process_group("gloo", rank=0, world_size=1)
+    cfg = CONFIGS[args.config]
+    L, T, mcs_per_step = cfg["L"], cfg["tile"], cfg["mcs_per_step"]
+    d = DistSlab(SlabHandle(L, cfg["p"], cfg["q"], T, cfg["seed"], world, rank, device=dev))
+    d.init_flat()
+    for _ in range(args.warmup):
+        d.run(mcs_per_step)
+        d.measure()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
+    t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)
+    t0.record()
+    last = None
+    for _ in range(args.steps):
+        d.run(mcs_per_step)
+        last = d.measure()
+    t1.record()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    sec = torch.tensor([t0.elapsed_time(t1) * 1e-3], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(sec, op=dist.ReduceOp.MAX)
+    sec = float(sec.item())
+    if rank == 0:
+        units = args.steps * mcs_per_step * L * L
+        print(json.dumps({"metric": METRIC, "value": units / sec / 1e9, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": sec / args.steps * 1e3, "higher_is_better": True,
+                          "scaling": "strong", "vs_baseline": None, "dtype": "u32 bit-logic + Philox4x32 (int32/int64 sums)",
+                          "data": "synthetic",
+                          "config": {"workload": cfg["name"], "L": L, "tile": T, "p": cfg["p"], "q": cfg["q"], "seed": cfg["seed"],
+                                     "mcs_per_step": mcs_per_step, "parallelism": "one lattice as %d slabs of rows" % world,
+                                     "step": "4 colour passes per MCS with ghost-row exchange + slab measurement"},
+                          "W2_last": last[2], "clocks": clocks, "e2e": None, "gpu_launches": None, "roofline": None,
+                          "cpu_baseline": None}))
+    dist.destroy_process_group()
+
+
 def _cpu_model():
     try:
         for line in open("/proc/cpuinfo"):
@@ -469,6 +529,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--pipeline", action="store_true", help="also time kpz_pipeline_host for configs other than 3")
     ap.add_argument("--peaks", action="store_true", help="print the pipe micro-benchmarks (kpz_measure_peaks) and exit")
+    ap.add_argument("--slabs", action="store_true", help="ONE lattice of the config split into slabs of rows over the N ranks "
+                                                         "(strong scaling; DESIGN.md Multi-GPU) instead of one lattice per rank")
     ap.add_argument("--launcher-selftest", action="store_true", help="multi-rank launch + reductions only (gloo, no GPU)")
     args = ap.parse_args()
     args.steps = args.steps or CONFIGS[args.config]["steps"]
@@ -480,6 +542,9 @@ def main():
         sys.exit(relaunch_under_torchrun(args))
     if args.launcher_selftest:
         launcher_selftest(args)
+        return
+    if args.slabs:
+        run_slabs(args)
         return
     if args.peaks:
         import paper_1110_6745_b200 as pkg

@@ -938,3 +938,28 @@ def test_slab_handles_validate_and_refuse_whole_lattice_calls(pkg):
     for m in (0, 1, 17, 2**32 - 2):
         assert tuple(h.global_draw(m)) == tuple(o.global_draw(m))      # host evaluation of S2 = the oracle's
     h.close()
+
+
+def test_dist_slab_single_rank_matches_oracle(pkg):
+    """DistSlab (the one-process-per-GPU driver) with the real CUDA slab handle in a group of one rank: the ghost rows
+    wrap onto the slab's own head; state sums and counters against the oracle.  (World sizes 2 and 4 of the same driver
+    run on CPU with a stand-in handle: tests/test_slabs_gloo.py.)"""
+    import socket
+    import torch.distributed as dist
+    from paper_1110_6745_b200.slabs import DistSlab, SlabHandle
+    L, T, p, q, seed = 512, 32, 0.75, 0.25, 91
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK="0", WORLD_SIZE="1")
+    dist.init_process_group("gloo", rank=0, world_size=1)
+    try:
+        d = DistSlab(SlabHandle(L, p, q, T, seed, 1, 0))
+        d.init_flat()
+        o = Oracle(L, p, q, T, seed, threads=NTHREADS)
+        o.init_flat()
+        for _ in range(3):
+            d.run(2); o.run(2)
+            assert d.measure() == o.measure()
+            assert d.h.counters() == o.counters()
+        d.h.close()
+    finally:
+        dist.destroy_process_group()
