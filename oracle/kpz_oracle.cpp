@@ -22,6 +22,8 @@
 // conservation + curl-free after every step, +2 per accepted flip, exact L=4 / L=6 Markov chains.
 // "parity unpinned" (definitions of this build, pinned only by the independent Python twin in
 // oracle/kpz_twin.py and by distribution tests): tile-colour order decode, offset draw, step -> Philox word map.
+// kpzo_state_hash is a checksum, not part of the method, and is "parity unpinned" as well (both sides restate the
+// formula of SURVEY 8(b)); no parity case relies on it alone.
 //
 // Optional OpenMP: tiles of one colour are independent,
 // so the tile loop may run in parallel; results are identical for any thread count.  The same holds for the
