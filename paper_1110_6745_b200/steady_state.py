@@ -61,7 +61,7 @@ def finite_size_scaling(results):
     """Finite-size scaling of a list of run() outputs of different L: alpha_eff(L) of eq. (13)
     between sizes L and L/2 from kappa_1 = <W^2> -- with the intrinsic 1/4 of the zig-zag start subtracted and
     without --, the power-law exponents of eq. (19) as alpha_n = s_n / (2 n) for the cumulants that are positive at
-    every size, and the fit of eq. (14) when at least three local slopes exist."""
+    every size, and the fit of eq. (14) when at least four local slopes exist (three parameters)."""
     results = sorted(results, key=lambda r: r["L"])
     sizes = [r["L"] for r in results]
     k1 = [r["cumulants"][0] for r in results]
@@ -74,7 +74,7 @@ def finite_size_scaling(results):
         if len(sizes) >= 2 and all(v > 0 for v in kn):
             c, sl = analysis.fit_power_law(sizes, kn)
             out["cumulant_power_laws"].append({"n": n, "prefactor": c, "exponent": sl, "alpha_n": sl / (2 * n)})
-    if len(out["alpha_eff"]) >= 3:
+    if len(out["alpha_eff"]) >= 4:
         f = analysis.fit_correction([a["L"] for a in out["alpha_eff"]], [a["alpha_eff"] for a in out["alpha_eff"]])
         out["eq14_fit"] = {"alpha": f["asymptote"], "a1": f["amplitude"], "omega1": f["exponent"], "rss": f["rss"]}
     return out

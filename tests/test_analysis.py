@@ -139,3 +139,4 @@ def test_finite_size_scaling_reduces_run_outputs():
     assert all(c["alpha_n"] == pytest.approx(alpha, abs=1e-12) for c in f["cumulant_power_laws"][1:])
     assert f["cumulant_power_laws"][0]["alpha_n"] < alpha               # kappa_1 still carries the additive 1/4
     assert "eq14_fit" in f
+    assert "eq14_fit" not in steady_state.finite_size_scaling(runs[:4])     # three slopes cannot fix three parameters
