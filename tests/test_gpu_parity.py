@@ -297,6 +297,26 @@ def test_replica_batch_parity(pkg):
     assert len({k.state_hash(r) for r in range(R)}) == R
 
 
+def test_config4_replicas_2000_mcs_in_one_launch(pkg):
+    """Config-4 shape over the run length S:8(d) asks for ("all replicas for the first 2 000 MCS"): 16 replicas of
+    L = 128, T = 16, p = 1, q = 0, seed 4 advanced 2 000 MCS by ONE launch of the lattice-resident kernel (the MCS clock
+    counts inside the kernel), then 7 more; sums, W^2, counters and hashes of every replica against the oracle."""
+    L, T, seed, R = 128, 16, 4, 16
+    k = pkg.KPZ(L, 1.0, 0.0, T, seed, n_replicas=R)
+    k.init_flat()
+    l0 = k.launch_count()
+    k.run(2000)
+    assert k.launch_count() - l0 == 1
+    k.run(7)
+    os_ = [Oracle(L, 1.0, 0.0, T, seed, replica=r) for r in range(R)]
+    for o in os_:
+        o.init_flat(); o.run(2007)
+    _compare_scalars(k, os_)
+    for r in range(R):
+        assert k.state_hash(r) == os_[r].state_hash()
+    _compare_full(k, os_[R - 1], replica=R - 1)
+
+
 def test_replica_batch_1024_general_pq(pkg):
     L, T, seed, R, n = 128, 16, 4, 1024, 3
     k = pkg.KPZ(L, 0.75, 0.25, T, seed, n_replicas=R)
