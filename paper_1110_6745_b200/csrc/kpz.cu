@@ -667,7 +667,7 @@ int32_t kpz_import_packed(kpz_ctx* c, const void* host_src, size_t bytes, const 
     KPZ_CUDA(c, cudaMemcpyAsync(c->d_scratch + c->sl.stats, st.data(), (size_t)c->R * 32, cudaMemcpyHostToDevice, c->stream));
     KPZ_CUDA(c, cudaStreamSynchronize(c->stream));
     c->mcs = mcs;
-    c->attempts_base = mcs * (uint64_t)c->L * c->L;
+    c->attempts_base = mcs * (uint64_t)c->L * c->rows_own;      // rows_own = L for a whole lattice
     return KPZ_OK;
 }
 
