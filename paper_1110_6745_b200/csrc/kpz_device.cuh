@@ -595,42 +595,6 @@ __device__ __forceinline__ void attempt(uint32_t* __restrict__ sm, uint32_t site
     }
 }
 
-#if defined(KPZ_SPEC2)
-// Variant (measured): two consecutive attempts of a tile evaluated together.  Both load their
-// five words before the first one's reduction, so the two chains overlap; the pair is exact unless the second site
-// lies within distance 1 of the first (then the first one's flip could change the second one's neighbourhood): those
-// lanes take the sequential path.  p = 1, q = 0, T >= 32 only.
-template <int T, int NTHR>
-__device__ __forceinline__ void attempt_pair(uint32_t* __restrict__ sm, uint32_t wA, uint32_t wB, float& dep_f) {
-    using G = TileGeom<T>;
-    const uint32_t iA = wA >> (32 - 2 * G::LOG2T), iB = wB >> (32 - 2 * G::LOG2T);
-    uint32_t* aA = sm + ((iA >> 5) + (iA >> G::LOG2T) + (uint32_t)(G::PAD + G::WPR)) * NTHR;
-    uint32_t* aB = sm + ((iB >> 5) + (iB >> G::LOG2T) + (uint32_t)(G::PAD + G::WPR)) * NTHR;
-    const int32_t d = (int32_t)iB - (int32_t)iA;
-    const uint32_t d2 = (uint32_t)(d * d);
-    const bool near = (d2 <= 1u) || (d2 == (uint32_t)(T * T));
-    const uint32_t bA = __funnelshift_l(0u, 1u, iA), bB = __funnelshift_l(0u, 1u, iB);
-    if (!near) {
-        const uint32_t oA = aA[0], pA = *(aA - NTHR), nA = aA[NTHR], dA = *(aA - G::WPR * NTHR), uA = aA[G::WPR * NTHR];
-        const uint32_t oB = aB[0], pB = *(aB - NTHR), nB = aB[NTHR], dB = *(aB - G::WPR * NTHR), uB = aB[G::WPR * NTHR];
-        const uint32_t mA = lop3_and_not_not(bA, lop3<0xDB>(oA, __funnelshift_l(pA, oA, 1), __funnelshift_r(oA, nA, 1)), lop3<0xBD>(oA, uA, dA));
-        const uint32_t mB = lop3_and_not_not(bB, lop3<0xDB>(oB, __funnelshift_l(pB, oB, 1), __funnelshift_r(oB, nB, 1)), lop3<0xBD>(oB, uB, dB));
-        atomicXor(aA, mA);
-        atomicXor(aB, mB);
-        asm("{ .reg .pred p; setp.ne.u32 p, %1, 0; @p add.f32 %0, %0, 0f3F800000; }" : "+f"(dep_f) : "r"(mA));
-        asm("{ .reg .pred p; setp.ne.u32 p, %1, 0; @p add.f32 %0, %0, 0f3F800000; }" : "+f"(dep_f) : "r"(mB));
-    } else {
-        const uint32_t oA = aA[0], pA = *(aA - NTHR), nA = aA[NTHR], dA = *(aA - G::WPR * NTHR), uA = aA[G::WPR * NTHR];
-        const uint32_t mA = lop3_and_not_not(bA, lop3<0xDB>(oA, __funnelshift_l(pA, oA, 1), __funnelshift_r(oA, nA, 1)), lop3<0xBD>(oA, uA, dA));
-        atomicXor(aA, mA);
-        const uint32_t oB = aB[0], pB = *(aB - NTHR), nB = aB[NTHR], dB = *(aB - G::WPR * NTHR), uB = aB[G::WPR * NTHR];
-        const uint32_t mB = lop3_and_not_not(bB, lop3<0xDB>(oB, __funnelshift_l(pB, oB, 1), __funnelshift_r(oB, nB, 1)), lop3<0xBD>(oB, uB, dB));
-        atomicXor(aB, mB);
-        asm("{ .reg .pred p; setp.ne.u32 p, %1, 0; @p add.f32 %0, %0, 0f3F800000; }" : "+f"(dep_f) : "r"(mA));
-        asm("{ .reg .pred p; setp.ne.u32 p, %1, 0; @p add.f32 %0, %0, 0f3F800000; }" : "+f"(dep_f) : "r"(mB));
-    }
-}
-#endif
 
 // T*T sequential attempts of one tile (S3).  Site call c serves steps 8c..8c+7: each of its four words is a
 // base-T*T fraction with two digits (for the power-of-two T*T of this path: its top 2*log2(T) bits and the next
@@ -670,16 +634,6 @@ __device__ __forceinline__ void run_tile_steps(uint32_t* __restrict__ sm, const 
         const uint32_t rem = n_steps - 8u * (c - c_begin);      // S7: live steps left in this call and after
         const uint4 a0 = MODE ? cur_a[0] : make_uint4(0u, 0u, 0u, 0u);
         const uint4 a1 = MODE ? cur_a[1] : make_uint4(0u, 0u, 0u, 0u);
-#if defined(KPZ_SPEC2)
-        if constexpr (MODE == 0 && !TRACK && !DEAD && SUBM == 0 && TileGeom<T>::WIDE) {
-            attempt_pair<T, NTHR>(sm, cur.x, cur.x * TT, dep_f);
-            attempt_pair<T, NTHR>(sm, cur.y, cur.y * TT, dep_f);
-            attempt_pair<T, NTHR>(sm, cur.z, cur.z * TT, dep_f);
-            attempt_pair<T, NTHR>(sm, cur.w, cur.w * TT, dep_f);
-            cur = nxt;
-            continue;
-        }
-#endif
         attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.x, a0.x, P, n_dep, dep_f, n_rem, rem_f, dh00, origin_idx, SUBM != 2 || rem > 0u);
         attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.x * TT, a0.y, P, n_dep, dep_f, n_rem, rem_f, dh00, origin_idx, SUBM != 2 || rem > 1u);
         attempt<T, NTHR, MODE, TRACK, DEAD>(sm, cur.y, a0.z, P, n_dep, dep_f, n_rem, rem_f, dh00, origin_idx, SUBM != 2 || rem > 2u);
