@@ -125,6 +125,26 @@ int32_t kpz_set_poisson(kpz_ctx* ctx, int32_t on);
  * Does not modify the lattice.  KPZ_EOVERFLOW if a requested sum does not fit int64 (W2 is still written). */
 int32_t kpz_measure(kpz_ctx* ctx, int64_t* sum_h, int64_t* sum_h2, double* W2);
 
+/* kpz_measure WITHOUT any allocation and without a host synchronisation, for callers that cannot allocate (code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): the partial sums of the measurement
+ * kernels live in a file-scope static device array of the library (819 456 bytes, held by every GPU that loads the
+ * library until exit) instead of the bound scratch buffer.  LIMIT: L <= 8192 (KPZ_STATIC_MAX_L; the paper's largest
+ * steady-state size); a larger handle gets KPZ_EINVAL and must use kpz_measure.
+ *   replica : which lattice of the handle (input: the handle's bound lattice and its tracked h(0,0), both on the device)
+ *   d_out   : caller-owned DEVICE buffer of 8 x 8 bytes, 8-byte aligned (output), written asynchronously on the bound
+ *             stream: [0..3] the four 64-bit half-accumulators (lo / hi of sum (h - h00), lo / hi of sum (h - h00)^2:
+ *             what kpz_slab_finalize takes), [4] sum h (int64), [5] sum h^2 (int64), [6] W^2 (double, the same
+ *             128-bit integer arithmetic as kpz_measure: identical bits), [7] 1 if a sum does not fit int64 (it is
+ *             then written as 0), else 0.
+ * Calls no cudaMalloc, cudaFree or allocating routine; enqueues one 32-byte memset and four kernels.  The first call on
+ * a device looks the array's address up (cudaGetSymbolAddress): make one call outside a graph capture first.
+ * ALL handles and calls of a process share the one array per device, and it keeps the last call's contents (the call
+ * clears what must start at zero): calls that may overlap on the GPU -- different streams, or graphs launched
+ * concurrently -- RACE; serialise them (one stream, or events).  Does not modify the lattice or the handle's state.
+ * Errors: KPZ_ESTATE (not bound, slab handle), KPZ_EINVAL (replica, d_out NULL / misaligned, L > 8192), KPZ_ECUDA. */
+#define KPZ_STATIC_MAX_L 8192
+int32_t kpz_measure_static(kpz_ctx* ctx, uint32_t replica, void* d_out);
+
 /* Sampling-time driver ("the program calculates and writes out the width" at the times t_i of eq. 8):
  * advances to each absolute MCS clock times[i] (HOST array, strictly increasing, times[0] >= the current clock)
  * and measures there.  HOST out-arrays of n_times * n_replicas entries, sample-major [i * n_replicas + r] (any may

@@ -24,7 +24,7 @@ exported_symbols = [
     "kpz_launch_count", "kpz_philox_selftest", "kpz_profiles", "kpz_power_spectrum", "kpz_set_schedule", "kpz_set_sub_sweeps", "kpz_run_sampled", "kpz_set_poisson",
     "kpz_set_path", "kpz_measure_peaks",
     "kpz_slab_workspace_bytes", "kpz_create_slab", "kpz_slab_info", "kpz_global_draw", "kpz_slab_pass", "kpz_slab_end_mcs",
-    "kpz_slab_measure_local", "kpz_slab_measure_finish", "kpz_slab_finalize",
+    "kpz_slab_measure_local", "kpz_slab_measure_finish", "kpz_slab_finalize", "kpz_measure_static",
 ]
 
 
@@ -83,6 +83,7 @@ def load_library() -> ctypes.CDLL:
         "kpz_slab_measure_local": [vp],
         "kpz_slab_measure_finish": [vp, vp, vp, vp],
         "kpz_slab_finalize": [u32, vp, i64, vp, vp, vp],
+        "kpz_measure_static": [vp, u32, vp],
     }
     for name, args in sig.items():
         fn = getattr(L, name)
@@ -177,6 +178,13 @@ class KPZ:
         w2 = np.zeros(R, dtype=np.float64)
         self._check(self._lib.kpz_measure(self._h, s1.ctypes.data, s2.ctypes.data, w2.ctypes.data))
         return s1, s2, w2
+
+    def measure_static(self, out, replica=0):
+        """kpz_measure_static: the measurement with its scratch in the library's static device array (no allocation, no
+        host synchronisation; L <= 8192).  `out` is the CALLER's device tensor of 8 int64 words (see include/kpz.h);
+        it is written asynchronously on the bound stream."""
+        assert out.is_cuda and out.numel() * out.element_size() >= 64 and out.is_contiguous()
+        self._check(self._lib.kpz_measure_static(self._h, replica, out.data_ptr()))
 
     def get_slopes(self, replica=0):
         sx = np.zeros((self.L, self.L), dtype=np.int8)

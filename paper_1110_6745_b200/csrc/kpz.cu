@@ -313,6 +313,60 @@ cudaError_t run_peak(uint32_t blocks, uint32_t iters, uint32_t* sink, unsigned l
     return e;
 }
 
+// ---- kpz_measure_static: the measurement with its scratch in a file-scope static array (no allocation) ----------
+// For callers that cannot allocate (code under CUDA graph capture, tight serving loops).  The partial sums of the
+// measurement kernels -- row-0 prefix, per-chunk (S0, S1, S2) of every column, the four 64-bit half-accumulators --
+// live in this array instead of the caller's scratch buffer.  Every GPU that loads the library holds it until exit.
+// Maximum lattice edge KPZ_STATIC_MAX_L = 8192 (include/kpz.h; the paper's largest steady-state size): 819 456 bytes.
+// Layout (bytes): [0, 256) four u64 half-accumulators; base[L_max] int32; cS0, cS1, cS2 [NC_max][L_max] int32 each.
+constexpr uint32_t KPZ_STATIC_MAX_CHUNKS = KPZ_STATIC_MAX_L / 1024;      // KPZ_STATIC_MAX_L: include/kpz.h
+constexpr size_t KPZ_STATIC_OFF_BASE = 256;
+constexpr size_t KPZ_STATIC_OFF_CS = KPZ_STATIC_OFF_BASE + (size_t)KPZ_STATIC_MAX_L * 4;
+constexpr size_t KPZ_STATIC_CS_BYTES = (size_t)KPZ_STATIC_MAX_CHUNKS * KPZ_STATIC_MAX_L * 4;
+constexpr size_t KPZ_STATIC_BYTES = KPZ_STATIC_OFF_CS + 3 * KPZ_STATIC_CS_BYTES;
+static __device__ __align__(256) unsigned char kpz_static_scratch[KPZ_STATIC_BYTES];
+
+// Device code may name the array directly.  One thread: half-accumulators -> sum h, sum h^2, W^2 (same 128-bit integer
+// arithmetic as the host's finalize_sums: R16) written to the caller's DEVICE buffer out[8]:
+//   [0..3] the half-accumulators (lo / hi of sum (h - h00), lo / hi of sum (h - h00)^2)
+//   [4] sum h (int64), [5] sum h^2 (int64), [6] W^2 (double), [7] 1 if a sum does not fit int64 (it is then 0) else 0
+__global__ void kpz_static_finalize_kernel(const unsigned long long* __restrict__ stats, uint32_t replica, uint32_t L,
+                                           unsigned long long* __restrict__ out) {
+    if (blockIdx.x != 0 || threadIdx.x != 0) return;
+    const unsigned long long* hm = reinterpret_cast<const unsigned long long*>(kpz_static_scratch);
+    const i128 S1 = (i128)(long long)hm[1] * ((i128)1 << 32) + (i128)hm[0];
+    const i128 S2 = (i128)(long long)hm[3] * ((i128)1 << 32) + (i128)hm[2];
+    const i128 h0 = (long long)stats[(size_t)replica * 4u + 2u];
+    const i128 N = (i128)L * L;
+    const double Nd = (double)((unsigned long long)L * L);
+    const i128 sh = S1 + N * h0;
+    const i128 sh2 = S2 + 2 * h0 * S1 + N * h0 * h0;
+    const i128 num = N * S2 - S1 * S1;
+    const i128 lo = -((i128)1 << 63), hi = ((i128)1 << 63) - 1;
+    const bool ok1 = sh >= lo && sh <= hi, ok2 = sh2 >= lo && sh2 <= hi;
+    out[0] = hm[0]; out[1] = hm[1]; out[2] = hm[2]; out[3] = hm[3];
+    out[4] = ok1 ? (unsigned long long)(long long)sh : 0ull;
+    out[5] = ok2 ? (unsigned long long)(long long)sh2 : 0ull;
+    out[6] = (unsigned long long)__double_as_longlong((double)num / (Nd * Nd));
+    out[7] = (ok1 && ok2) ? 0ull : 1ull;
+}
+
+// In host code the array's name is a host-side stand-in, not a device address: look the address up once per device,
+// with that device current, and hand THAT to the kernels.
+int32_t static_scratch_ptr(kpz_ctx* c, unsigned char** out) {
+    static unsigned char* ptr[KPZ_MAX_DEVICES] = {};
+    const int dev = c->device;
+    if (dev < 0 || dev >= KPZ_MAX_DEVICES) return kpz_fail(c, KPZ_ESTATE, "handle has no device");
+    if (!ptr[dev]) {
+        unsigned char* p = nullptr;
+        KPZ_CUDA(c, cudaGetSymbolAddress((void**)&p, kpz_static_scratch));      // the caller made `dev` current
+        if (!p) return kpz_fail(c, KPZ_ECUDA, "cudaGetSymbolAddress returned a NULL address");
+        ptr[dev] = p;
+    }
+    *out = ptr[dev];
+    return KPZ_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -497,6 +551,47 @@ int32_t kpz_measure(kpz_ctx* c, int64_t* sum_h, int64_t* sum_h2, double* W2) {
         overflow |= finalize_sums(c->L, S1[r], S2[r], h00[r], sum_h ? sum_h + r : nullptr, sum_h2 ? sum_h2 + r : nullptr,
                                   W2 ? W2 + r : nullptr);
     if (overflow) return kpz_fail(c, KPZ_EOVERFLOW, "a sum does not fit int64");
+    return KPZ_OK;
+}
+
+int32_t kpz_measure_static(kpz_ctx* c, uint32_t replica, void* d_out) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
+    if ((rc = require_whole(c)) != KPZ_OK) return rc;
+    if (replica >= c->R) return kpz_fail(c, KPZ_EINVAL, "replica out of range");
+    if (!d_out || ((uintptr_t)d_out & 7u)) return kpz_fail(c, KPZ_EINVAL, "d_out must be an 8-byte aligned DEVICE pointer to 64 bytes");
+    if (c->L > KPZ_STATIC_MAX_L)
+        return kpz_fail(c, KPZ_EINVAL, "kpz_measure_static: L = %u exceeds the static scratch maximum of L = %u (use kpz_measure)",
+                        c->L, (uint32_t)KPZ_STATIC_MAX_L);
+    unsigned char* sp = nullptr;
+    if ((rc = static_scratch_ptr(c, &sp)) != KPZ_OK) return rc;
+    const uint32_t L = c->L, W = L / 32;
+    const uint64_t plane_words = (uint64_t)L * L / 32;
+    const uint32_t* lat = c->d_lattice + (size_t)replica * 2u * plane_words;      // this replica's two planes
+    unsigned long long* msum = reinterpret_cast<unsigned long long*>(sp);
+    int32_t* base = reinterpret_cast<int32_t*>(sp + KPZ_STATIC_OFF_BASE);
+    int32_t* cS0 = reinterpret_cast<int32_t*>(sp + KPZ_STATIC_OFF_CS);
+    int32_t* cS1 = reinterpret_cast<int32_t*>(sp + KPZ_STATIC_OFF_CS + KPZ_STATIC_CS_BYTES);
+    int32_t* cS2 = reinterpret_cast<int32_t*>(sp + KPZ_STATIC_OFF_CS + 2 * KPZ_STATIC_CS_BYTES);
+    // the array keeps the last call's contents: the accumulators must start at zero (base and the chunk partials are
+    // overwritten in full for this L before they are read)
+    KPZ_CUDA(c, cudaMemsetAsync(msum, 0, 32, c->stream));
+    int nthr = 1024;
+    while (nthr > 32 && (uint32_t)nthr > L) nthr >>= 1;
+    kpz::kpz_row0_prefix_kernel<<<1, nthr, 0, c->stream>>>(lat, plane_words, L, W, base);
+    KPZ_CUDA(c, cudaGetLastError());
+    dim3 g1((W + 127) / 128, c->sl.n_chunks, 1);
+    kpz::kpz_column_chunk_kernel<<<g1, 128, 0, c->stream>>>(lat, plane_words, L, W, c->sl.rows_per_chunk, cS0, cS1, cS2, L, 1u);
+    KPZ_CUDA(c, cudaGetLastError());
+    dim3 g2((L + 255) / 256, 1);
+    kpz::kpz_combine_kernel<<<g2, 256, 0, c->stream>>>(base, cS0, cS1, cS2, L, c->sl.n_chunks, c->sl.rows_per_chunk, msum, nullptr,
+                                                    0u, L);
+    KPZ_CUDA(c, cudaGetLastError());
+    kpz_static_finalize_kernel<<<1, 32, 0, c->stream>>>(reinterpret_cast<const unsigned long long*>(c->d_scratch + c->sl.stats), replica,
+                                                     L, static_cast<unsigned long long*>(d_out));
+    KPZ_CUDA(c, cudaGetLastError());
+    c->launches += 4;
     return KPZ_OK;
 }
 
