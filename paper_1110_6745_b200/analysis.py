@@ -2,6 +2,7 @@
 
 Nothing here runs on the hot path: these are the few scalar formulas the paper applies to the measured widths.
   * cumulants           -- eq. (18): kappa_1..kappa_4 from the non-central moments nu_n of W^2
+  * pool_cumulants      -- eq. (18) over the union of several batches (moments pool as weighted averages)
   * width_distribution  -- Psi_L(x) = <W^2> P_L(W^2 / <W^2>), as a normalised histogram
   * steady_state_t_end  -- run length of BASELINE config 4: t = 20 L^1.61 MCS, rounded up
   * sampling_times      -- eq. (8): t_{i+1} = (t_i + 10) e^m, t_0 = 0, as distinct integers floor(t_i)
@@ -39,6 +40,28 @@ def cumulants(w2):
     k3 = n3 - 3.0 * n1 * n2 + 2.0 * n1 ** 3
     k4 = n4 - 4.0 * n3 * n1 - 3.0 * n2 ** 2 + 12.0 * n1 ** 2 * n2 - 6.0 * n1 ** 4
     return k1, k2, k3, k4
+
+
+def moments_from_cumulants(k):
+    """Inverse of eq. (18): (nu_1..nu_4) from (kappa_1..kappa_4)."""
+    k1, k2, k3, k4 = k
+    n1 = k1
+    n2 = k2 + k1 ** 2
+    n3 = k3 + 3.0 * n1 * n2 - 2.0 * n1 ** 3
+    n4 = k4 + 4.0 * n3 * n1 + 3.0 * n2 ** 2 - 12.0 * n1 ** 2 * n2 + 6.0 * n1 ** 4
+    return n1, n2, n3, n4
+
+
+def pool_cumulants(batches):
+    """Cumulants of the union of several batches of samples, each given as (n_samples, (kappa_1..kappa_4)): the
+    non-central moments of eq. (18) are plain averages, so they pool with the sample counts as weights.  For
+    ensembles run as several independent batches (e.g. config 4's 256 replicas of L = 2048 as four runs of 64)."""
+    n_tot = float(sum(n for n, _ in batches))
+    nu = [sum(n * m for n, m in zip([b[0] for b in batches], col)) / n_tot
+          for col in zip(*[moments_from_cumulants(k) for _, k in batches])]
+    n1, n2, n3, n4 = nu
+    return (n1, n2 - n1 ** 2, n3 - 3.0 * n1 * n2 + 2.0 * n1 ** 3,
+            n4 - 4.0 * n3 * n1 - 3.0 * n2 ** 2 + 12.0 * n1 ** 2 * n2 - 6.0 * n1 ** 4)
 
 
 def width_distribution(w2, bins=50, x_range=(0.0, 3.0)):

@@ -140,3 +140,16 @@ def test_finite_size_scaling_reduces_run_outputs():
     assert f["cumulant_power_laws"][0]["alpha_n"] < alpha               # kappa_1 still carries the additive 1/4
     assert "eq14_fit" in f
     assert "eq14_fit" not in steady_state.finite_size_scaling(runs[:4])     # three slopes cannot fix three parameters
+
+
+def test_pool_cumulants_equals_cumulants_of_the_union():
+    """eq. (18) on batches: pooling (n, cumulants) of three unequal batches reproduces the cumulants of all samples
+    together, and the inversion cumulants -> moments is exact on a rational example."""
+    rng = np.random.default_rng(8)
+    parts = [rng.gamma(7.0, 1.3, n) for n in (6400, 19200, 1000)]
+    pooled = analysis.pool_cumulants([(len(p), analysis.cumulants(p)) for p in parts])
+    direct = analysis.cumulants(np.concatenate(parts))
+    for a, b in zip(pooled, direct):
+        assert a == pytest.approx(b, rel=1e-9)
+    vals = [0, 1, 1, 3]                                    # nu = 5/4, 11/4, 29/4, 83/4
+    assert analysis.moments_from_cumulants(analysis.cumulants(vals)) == pytest.approx((1.25, 2.75, 7.25, 20.75), rel=1e-12)
