@@ -7,6 +7,10 @@ the cumulants kappa_1..kappa_4 (eq. 18), the width distribution Psi_L(x) and the
                                                   [--sub-sweeps K] [--spectrum-replicas 8] [--peaks]
     python -m paper_1110_6745_b200.steady_state --sizes 128,256,512,1024 --replicas 1024,256,256,256
         (finite-size scaling over several sizes: alpha_eff(L) of eq. 13, the power laws of eq. 19 for kappa_1..kappa_4)
+    python -m paper_1110_6745_b200.steady_state --pool batch1.json batch2.json ... [--fss-with runs.json]
+        (no GPU: pools the cumulants of several independent batches of ONE size -- outputs of this program, e.g. config
+        4's 256 replicas of L = 2048 run as four batches of 64 under different Philox keys -- and, with --fss-with, adds
+        the pooled size to the runs of a --sizes output and repeats the finite-size scaling)
 """
 from __future__ import annotations
 
@@ -80,6 +84,18 @@ def finite_size_scaling(results):
     return out
 
 
+def pool_batches(batches):
+    """Several run() outputs (or {"L", "replicas", "n_samples", "cumulants"} records) of ONE lattice size -> one record
+    with the cumulants of the union of their samples (analysis.pool_cumulants)."""
+    sizes = {b["L"] for b in batches}
+    if len(sizes) != 1:
+        raise ValueError("batches of different lattice sizes cannot be pooled")
+    return {"L": sizes.pop(), "replicas": sum(b["replicas"] for b in batches),
+            "n_samples": sum(b["n_samples"] for b in batches), "seeds": [b.get("seed") for b in batches],
+            "t_end": batches[0].get("t_end"),
+            "cumulants": list(analysis.pool_cumulants([(b["n_samples"], b["cumulants"]) for b in batches]))}
+
+
 def schedule_peaks(S, L, tile):
     """S(k) at the mode numbers where the four-colour schedule leaves its imprint (odd multiples of L / (2 tile), and
     L / 4), each beside the median of its 12 neighbouring modes (profiles/r01_config4_steady.md, addendum)."""
@@ -104,7 +120,17 @@ def main():
     ap.add_argument("--spectrum-replicas", type=int, default=8)
     ap.add_argument("--peaks", action="store_true", help="print only S(k) at the schedule's peak modes")
     ap.add_argument("--sizes", type=str, default=None, help="comma-separated L: run every size, then finite_size_scaling")
+    ap.add_argument("--pool", nargs="+", default=None, help="JSON outputs of batches of one size: pool them (no GPU)")
+    ap.add_argument("--fss-with", type=str, default=None, help="with --pool: a --sizes output whose runs join the pooled size")
     args = ap.parse_args()
+    if args.pool:
+        pooled = pool_batches([json.load(open(f)) for f in args.pool])
+        out = {"pooled": pooled}
+        if args.fss_with:
+            runs = [r for r in json.load(open(args.fss_with))["runs"] if r["L"] != pooled["L"]] + [pooled]
+            out["fss"] = finite_size_scaling(runs)
+        print(json.dumps(out))
+        return
     if args.sizes:
         sizes = [int(v) for v in args.sizes.split(",")]
         reps = [int(v) for v in str(args.replicas).split(",")] if isinstance(args.replicas, str) else [args.replicas]

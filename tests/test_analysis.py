@@ -153,3 +153,25 @@ def test_pool_cumulants_equals_cumulants_of_the_union():
         assert a == pytest.approx(b, rel=1e-9)
     vals = [0, 1, 1, 3]                                    # nu = 5/4, 11/4, 29/4, 83/4
     assert analysis.moments_from_cumulants(analysis.cumulants(vals)) == pytest.approx((1.25, 2.75, 7.25, 20.75), rel=1e-12)
+
+
+def test_pool_batches_and_fss_with_the_pooled_size():
+    """steady_state.pool_batches: four batches of one size pool to the cumulants of all their samples; a pooled size
+    joins the other sizes in the finite-size scaling; sizes cannot be mixed."""
+    from paper_1110_6745_b200 import steady_state
+    rng = np.random.default_rng(9)
+    parts = [rng.gamma(9.0, 5.6, 6400) for _ in range(4)]
+    batches = [{"L": 2048, "replicas": 64, "seed": 4 + i, "n_samples": p.size, "cumulants": list(analysis.cumulants(p))}
+               for i, p in enumerate(parts)]
+    pooled = steady_state.pool_batches(batches)
+    assert pooled["replicas"] == 256 and pooled["n_samples"] == 25600 and pooled["seeds"] == [4, 5, 6, 7]
+    for a, b in zip(pooled["cumulants"], analysis.cumulants(np.concatenate(parts))):
+        assert a == pytest.approx(b, rel=1e-9)
+    alpha = 0.39
+    runs = [{"L": L, "cumulants": [0.25 + 0.15 * L ** (2 * alpha), 1.0, 1.0, 1.0]} for L in (128, 256, 512, 1024)]
+    big = dict(pooled, cumulants=[0.25 + 0.15 * 2048 ** (2 * alpha), 1.0, 1.0, 1.0])
+    f = steady_state.finite_size_scaling(runs + [big])
+    assert [a["L"] for a in f["alpha_eff"]] == [256, 512, 1024, 2048] and "eq14_fit" in f
+    assert all(a["alpha_eff"] == pytest.approx(alpha, abs=1e-12) for a in f["alpha_eff"])
+    with pytest.raises(ValueError):
+        steady_state.pool_batches(batches + [dict(batches[0], L=1024)])
