@@ -116,7 +116,8 @@ def fit_correction(x, y, exponent_range=(-4.0, -0.05), weights=None):
     """Least-squares fit of y(x) = y_inf + c1 e x^e (eq. 12: x = t, y = beta_eff, y_inf = beta, c1 = b1, e = phi1;
     eq. 14: x = L, y = alpha_eff, y_inf = alpha, c1 = a1, e = omega1; e signed, see the module docstring).
     For a fixed e the model is linear in (y_inf, c1 e): the exponent is found by a bounded 1-D search over the
-    profiled residual.  Returns {"asymptote", "amplitude" (= c1), "exponent", "rss"}."""
+    profiled residual.  Returns {"asymptote", "amplitude" (= c1), "exponent", "rss", "at_bound"}; at_bound = the exponent
+    ran into the edge of exponent_range, i.e. the correction is not resolved by the data."""
     from scipy.optimize import minimize_scalar
     x = np.asarray(x, dtype=np.float64)
     y = np.asarray(y, dtype=np.float64)
@@ -137,7 +138,10 @@ def fit_correction(x, y, exponent_range=(-4.0, -0.05), weights=None):
     res = minimize_scalar(lambda e: solve(e)[1], bounds=(lo, hi), method="bounded", options={"xatol": 1e-10})
     e = float(res.x)
     coef, r = solve(e)
-    return {"asymptote": float(coef[0]), "amplitude": float(coef[1]) / e, "exponent": e, "rss": r}
+    # an exponent on the edge of the search range means the data do not resolve the correction term (e.g. local slopes
+    # that are flat within their noise): only the asymptote is meaningful then
+    at_bound = min(abs(e - exponent_range[0]), abs(e - exponent_range[1])) < 1e-3 * (exponent_range[1] - exponent_range[0])
+    return {"asymptote": float(coef[0]), "amplitude": float(coef[1]) / e, "exponent": e, "rss": r, "at_bound": bool(at_bound)}
 
 
 def fit_power_law(x, y):

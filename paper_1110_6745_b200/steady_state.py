@@ -80,7 +80,11 @@ def finite_size_scaling(results):
             out["cumulant_power_laws"].append({"n": n, "prefactor": c, "exponent": sl, "alpha_n": sl / (2 * n)})
     if len(out["alpha_eff"]) >= 4:
         f = analysis.fit_correction([a["L"] for a in out["alpha_eff"]], [a["alpha_eff"] for a in out["alpha_eff"]])
-        out["eq14_fit"] = {"alpha": f["asymptote"], "a1": f["amplitude"], "omega1": f["exponent"], "rss": f["rss"]}
+        out["eq14_fit"] = {"alpha": f["asymptote"], "a1": f["amplitude"], "omega1": f["exponent"], "rss": f["rss"],
+                           "correction_resolved": not f["at_bound"]}
+        vals = [a["alpha_eff"] for a in out["alpha_eff"]]
+        out["alpha_eff_mean"] = float(np.mean(vals))
+        out["alpha_eff_spread"] = float(np.std(vals, ddof=1))
     return out
 
 

@@ -104,6 +104,9 @@ def test_alpha_eff_eq13_and_fit_eq14():
     Ls = np.array(sizes, dtype=np.float64)
     f = analysis.fit_correction(Ls, alpha + a1 * om * Ls ** om)
     assert (f["asymptote"], f["amplitude"], f["exponent"]) == pytest.approx((alpha, a1, om), rel=1e-6)
+    assert f["at_bound"] is False
+    flat = analysis.fit_correction(Ls, alpha + 1e-3 * (-1.0) ** np.arange(Ls.size))      # no trend: not resolvable
+    assert flat["at_bound"] is True and flat["asymptote"] == pytest.approx(alpha, abs=2e-3)
     with pytest.raises(ValueError):
         analysis.fit_correction([1, 2], [1, 2])
 

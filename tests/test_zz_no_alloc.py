@@ -112,3 +112,32 @@ def test_measure_static_rejects_what_it_cannot_hold(pkg):
     lib.kpz_destroy(h)
     _check(pkg, k, out, 0)                                             # and the handle still works after the refusals
     k.close()
+
+
+def test_measure_static_replays_inside_a_cuda_graph(pkg):
+    """What the entry point is for: captured once into a CUDA graph (one memset + four kernels, no allocation, no host
+    synchronisation), it is replayed after the lattice has moved on and gives kpz_measure's numbers each time.  (Only
+    the measurement is captured: kpz_run bakes the MCS clock into its launches and is issued normally, on the same
+    stream, between the replays.)"""
+    import torch
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        k = pkg.KPZ(512, 0.75, 0.25, 32, 21, stream=s)                 # the handle's stream is the capturing stream
+        out = torch.empty(8, dtype=torch.int64, device=k.device)
+        k.init_flat()
+        k.run(2)
+        k.measure_static(out)                                          # first call outside the capture: address lookup
+        s.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            k.measure_static(out)
+        for n in (0, 1, 3):
+            k.run(n)
+            out.fill_(-1)
+            g.replay()
+            s.synchronize()
+            w = [int(v) for v in out.cpu().tolist()]
+            s1, s2, w2 = k.measure()
+            assert (w[4], w[5], struct.unpack("<d", struct.pack("<q", w[6]))[0], w[7]) == \
+                (int(s1[0]), int(s2[0]), float(w2[0]), 0)
+        k.close()
