@@ -13,12 +13,17 @@ import json
 import math
 import time
 
+from . import analysis
 from .binding import KPZ
+
+
+T_MIC = 50      # "we disregarded the initial time region t < t_mic ~ 50"
 
 
 def sampling_times(t_max):
     """{1,2,5}*10^n (reading R15 for config 3) merged with the powers of two that beta_eff needs."""
     ts = {m * 10 ** n for n in range(0, 12) for m in (1, 2, 5)} | {2 ** i for i in range(0, 40)}
+    ts |= {25 * 10 ** n for n in range(0, 12)}       # the t/2 partners of 5 * 10^(n+1): every decade time has one
     return sorted(t for t in ts if t <= t_max)
 
 
@@ -37,8 +42,16 @@ def run(L, tile, p=1.0, q=0.0, seed=42, t_max=10000, device="cuda:0", every=Fals
         w = {r["t"]: r["W2"] - 0.25 for r in rows}
         beta = [{"t": t, "beta_eff": 0.5 * math.log2(w[t] / w[t // 2])} for t in times
                 if t >= 4 and (t & (t - 1)) == 0 and w[t // 2] > 0]
+        # eq. 11 on every sampled pair (t, t/2), and the correction fit of eq. 12 beyond t_mic ~ 50
+        slopes = [(t, b) for t, b in analysis.beta_eff(times, [r["W2"] for r in rows]) if t > T_MIC]
+        fit = None
+        if len(slopes) >= 4:
+            f = analysis.fit_correction([t for t, _ in slopes], [b for _, b in slopes])
+            fit = {"beta": f["asymptote"], "b1": f["amplitude"], "phi1": f["exponent"], "rss": f["rss"],
+                   "correction_resolved": not f["at_bound"], "n_points": len(slopes), "t_min": slopes[0][0]}
         n = L * L
-        return {"L": L, "tile": tile, "p": p, "q": q, "seed": seed, "samples": rows, "beta_eff": beta, "counters": c,
+        return {"L": L, "tile": tile, "p": p, "q": q, "seed": seed, "samples": rows, "beta_eff": beta, "eq12_fit": fit,
+                "counters": c,
                 "invariant_sum_h": int(s1[-1, 0]) == n // 2 + 2 * (c["deposits"] - c["removals"]),
                 "wall_s": wall, "gupds_incl_measurements": n * times[-1] / wall / 1e9}
     finally:

@@ -56,7 +56,7 @@ def test_config4_run_lengths_and_eq8_sampling_times():
 
 def test_growth_sampling_times():
     from paper_1110_6745_b200 import growth_run
-    assert growth_run.sampling_times(64) == [1, 2, 4, 5, 8, 10, 16, 20, 32, 50, 64]
+    assert growth_run.sampling_times(64) == [1, 2, 4, 5, 8, 10, 16, 20, 25, 32, 50, 64]
     ts = growth_run.sampling_times(10000)
     assert ts[-1] == 10000 and all(t in ts for t in (1, 2, 5, 10, 20, 50, 100, 200, 500, 1000, 2000, 5000, 8192))
     assert ts == sorted(set(ts))
