@@ -82,7 +82,7 @@ int32_t kpz_run(kpz_ctx* ctx, uint64_t mcs);
 
 /* Chooses the kernels kpz_run uses; the results are bit-identical on every path:
  *   KPZ_PATH_AUTO (default): the lattice-resident kernel when the packed lattice fits in shared memory (L <= 512),
- *     the schedule is the default S4 without sub-sweeps or Poissonised counts and the handle is small enough to
+ *     the schedule is S4, with or without sub-sweeps (S6), without Poissonised counts, and the handle is small enough to
  *     be bound by launches and tile staging; else the tiled kernel;
  *   KPZ_PATH_TILED: kpz_update_kernel, one launch per colour pass (4 per MCS), any valid L;
  *   KPZ_PATH_RESIDENT: force the resident kernel (one launch per kpz_run call, the lattices of a CTA's replicas

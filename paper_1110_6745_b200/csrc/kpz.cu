@@ -148,7 +148,7 @@ ResidentPlan resident_plan(const kpz_ctx* c) {
     const uint32_t L = c->L, T = c->T;
     const size_t lat = (size_t)L * L / 4;                        // bytes of one packed lattice
     const uint32_t HN = L / T / 2, tpc = HN * HN;
-    pl.ok = c->schedule == KPZ_SCHEDULE_COLOURS && c->sub_sweeps == 1 && !c->poisson && lat <= KPZ_RESIDENT_SMEM_MAX;
+    pl.ok = c->schedule == KPZ_SCHEDULE_COLOURS && !c->poisson && lat <= KPZ_RESIDENT_SMEM_MAX;      // S4, S6
     if (!pl.ok) return pl;
     // threads per CTA: a multiple of 128 wherever the handle has the tiles for it.  Warps are bound to the four
     // schedulers of an SM by their index inside the CTA, so single-warp CTAs would pile every chain of an SM onto

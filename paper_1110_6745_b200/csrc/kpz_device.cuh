@@ -768,7 +768,7 @@ __global__ void __launch_bounds__(NTHR, (T == 64) ? 3 : (T == 32 ? 8 : 1)) kpz_u
 // them -- the four colour passes of an MCS separated by __syncthreads() instead of kernel launches, the global
 // draw S2 evaluated in-kernel every pass -- and copies the lattices back.  Every step of a pass is the code of
 // kpz_update_kernel itself (stage_in_*, run_tile_steps, stage_out_* with the plane pointers aimed at shared memory),
-// so the trajectory is the tiled kernel's bit for bit; what disappears is the 4 launches per MCS and the global-
+// so the trajectory is the tiled kernel's bit for bit (schedules S4 and S6); what disappears is the 4 launches per MCS and the global-
 // memory round trips of the tile staging, which dominate when a colour has only a few hundred tiles.
 // Shared memory: [G][2][L*L/32] lattice words, then TileGeom<T>::WORDS * NTHR words of per-thread tiles.
 // STS = true: a flip is written with a plain store of the new word instead of an XOR reduction (the tile words
@@ -776,7 +776,7 @@ __global__ void __launch_bounds__(NTHR, (T == 64) ? 3 : (T == 32 ? 8 : 1)) kpz_u
 // ------------------------------------------------------------------------------------------------------------
 template <int T, int NTHR, int MODE>
 __global__ void __launch_bounds__(NTHR) kpz_resident_kernel(const UpdateParams P0, const uint32_t G, const uint32_t n_mcs,
-                                                            const uint32_t n_replicas) {
+                                                            const uint32_t n_replicas, const uint32_t n_sub) {
     using Geo = TileGeom<T>;
     extern __shared__ uint32_t smem[];
     const uint32_t g0 = blockIdx.x * G;
@@ -794,6 +794,14 @@ __global__ void __launch_bounds__(NTHR) kpz_resident_kernel(const UpdateParams P
     UpdateParams P = P0;
     for (uint32_t mi = 0; mi < n_mcs; ++mi) {
         P.m = P0.m + mi;
+        // S6: n_sub sub-sweeps per MCS, each with its own global draw and its slice of every tile's site calls
+        // (n_sub = 1: the whole stream, compile-time trip count).  Staging comes from shared memory here, so a
+        // sub-sweep costs little more than its attempts.
+        for (uint32_t sub = 0; sub < n_sub; ++sub) {
+        const uint32_t per = (uint32_t)(T * T / 8) / n_sub;
+        P.sub = sub;
+        P.call_begin = sub * per;
+        P.call_end = (sub + 1u) * per;
         for (uint32_t slot = 0; slot < 4u; ++slot) {
             P.slot = slot;
             for (uint32_t base = 0; base < items; base += NTHR) {
@@ -804,7 +812,7 @@ __global__ void __launch_bounds__(NTHR) kpz_resident_kernel(const UpdateParams P
                 const uint32_t replica = g0 + g;
                 const uint32_t j = wl / P0.HN, i = wl - j * P0.HN;
                 uint32_t ox, oy, colour;
-                global_draw<T>(P, 0u, replica, ox, oy, colour);
+                global_draw<T>(P, sub, replica, ox, oy, colour);
                 const uint32_t tx = 2u * i + (colour & 1u), ty = 2u * j + (colour >> 1);
                 const uint32_t X0 = ox + tx * T, Y0 = oy + ty * T;
                 const uint32_t tile_id = ty * P0.NT + tx;
@@ -824,10 +832,15 @@ __global__ void __launch_bounds__(NTHR) kpz_resident_kernel(const UpdateParams P
                 }
                 const bool any_origin = __any_sync(0xFFFFFFFFu, origin_idx != 0xFFFFFFFFu);
                 if (active) {
-                    if (any_origin)
-                        run_tile_steps<T, NTHR, MODE, true, false, 0>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx, 0u);
-                    else
-                        run_tile_steps<T, NTHR, MODE, false, false, 0>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx, 0u);
+                    if (n_sub == 1u) {
+                        if (any_origin)
+                            run_tile_steps<T, NTHR, MODE, true, false, 0>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx, 0u);
+                        else
+                            run_tile_steps<T, NTHR, MODE, false, false, 0>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx, 0u);
+                    } else {
+                        // TRACK = true is correct for every tile (it only adds the origin test): one instance less
+                        run_tile_steps<T, NTHR, MODE, true, false, 1>(sm, P, tile_id, replica, n_dep, n_rem, dh00, origin_idx, 0u);
+                    }
                     if constexpr (Geo::WIDE) stage_out_wide<T, NTHR, StageBatch<T>::N, false>(planeX, planeY, L, W, x0, y0, sm);
                     else stage_out_narrow<T, NTHR, false>(planeX, planeY, L, W, x0, y0, sm);
                     unsigned long long* st = P0.stats + (size_t)replica * 4u;
@@ -837,6 +850,7 @@ __global__ void __launch_bounds__(NTHR) kpz_resident_kernel(const UpdateParams P
                 }
             }
             __syncthreads();
+        }
         }
     }
     {

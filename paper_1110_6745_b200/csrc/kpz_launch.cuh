@@ -52,7 +52,7 @@ int32_t launch_resident_k(kpz_ctx* c, const kpz::UpdateParams& P, const Resident
         KPZ_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)KPZ_RESIDENT_SMEM_MAX));
         attr_set[dev] = true;
     }
-    kern<<<pl.blocks, NTHR, pl.smem, c->stream>>>(P, pl.G, n_mcs, c->R);
+    kern<<<pl.blocks, NTHR, pl.smem, c->stream>>>(P, pl.G, n_mcs, c->R, c->sub_sweeps);
     KPZ_CUDA(c, cudaGetLastError());
     c->launches++;
     return KPZ_OK;

@@ -218,6 +218,37 @@ def test_resident_paths_parity(pkg, path, L, T, p, q, seed, R, n):
     _compare_full(k, os_[R - 1], replica=R - 1)
 
 
+@pytest.mark.parametrize("L,T,p,q,K,R,seed", [
+    (64, 8, 1.0, 0.0, 2, 3, 46),
+    (128, 16, 1.0, 0.0, 4, 6, 47),             # config-4 shape with the knob that removes the S(k) peaks
+    (128, 16, 0.75, 0.25, 32, 2, 48),          # one site call per tile and sub-sweep
+    (256, 32, 0.6, 0.2, 8, 1, 49),
+    (512, 64, 1.0, 0.0, 16, 1, 50),
+])
+def test_resident_path_sub_sweeps_parity(pkg, L, T, p, q, K, R, seed):
+    """Schedule S6 through the lattice-resident kernel (every sub-sweep draws its own origin and colour order; all of
+    them inside ONE launch): state, sums, counters against the oracle, and against the tiled kernel."""
+    k = pkg.KPZ(L, p, q, T, seed, n_replicas=R)
+    k.set_path("resident"); k.set_sub_sweeps(K)
+    k.init_flat()
+    os_ = [Oracle(L, p, q, T, seed, replica=r, threads=NTHREADS) for r in range(R)]
+    for o in os_:
+        o.set_sub_sweeps(K); o.init_flat()
+    for n in (1, 3):
+        l0 = k.launch_count()
+        k.run(n)
+        assert k.launch_count() - l0 == 1
+        for o in os_:
+            o.run(n)
+        _compare_scalars(k, os_)
+        for r in range(R):
+            _compare_full(k, os_[r], replica=r)
+    t = pkg.KPZ(L, p, q, T, seed, n_replicas=R)
+    t.set_path("tiled"); t.set_sub_sweeps(K)
+    t.init_flat(); t.run(4)
+    assert [t.state_hash(r) for r in range(R)] == [k.state_hash(r) for r in range(R)]
+
+
 def test_resident_path_is_refused_when_it_cannot_hold_the_lattice(pkg):
     for (L, T, path) in ((2048, 16, "resident"), (1024, 64, "resident")):
         k = pkg.KPZ(L, 1.0, 0.0, T, 1)
@@ -233,10 +264,10 @@ def test_resident_path_is_refused_when_it_cannot_hold_the_lattice(pkg):
         assert k.state_hash() == o.state_hash()
     k = pkg.KPZ(128, 1.0, 0.0, 16, 1)
     k.set_path("resident")
-    k.set_sub_sweeps(2)
+    k.set_schedule("dead_border")
     k.init_flat()
     with pytest.raises(pkg.KpzError):
-        k.run(1)                                   # sub-sweeps run on the tiled kernel only
+        k.run(1)                                   # the dead-border schedule runs on the tiled kernel only
     with pytest.raises(KeyError):
         k.set_path("nonsense")
 
