@@ -200,6 +200,7 @@ def run_ours(args):
     # Local timings first; the reductions over ranks come after the try block, so that a rank whose pinned
     # allocation fails still takes part in them (a leg that failed on any rank is reported as unavailable).
     serial = (0.0, float("inf"))
+    overl = (0.0, float("inf"))
     piped = (0.0, float("inf"))
     n_e2e = max(1, min(args.steps, 3))
     n_rounds = max(3, (args.steps + 1) // 2)      # at least 6 pipelined steps, so that fill and drain do not dominate
@@ -218,6 +219,16 @@ def run_ours(args):
             mcs_now += mcs_per_step
         torch.cuda.synchronize()
         serial = (n_e2e * att_per_step, time.perf_counter() - w0)
+        # the same steps with the copies of the ONE lattice overlapped with its kernels slab by slab
+        k.step_host_overlapped(host, h00, mcs_now, mcs_per_step, args.e2e_slabs)       # warm-up
+        mcs_now += mcs_per_step
+        torch.cuda.synchronize()
+        w0 = time.perf_counter()
+        for _ in range(n_e2e):
+            k.step_host_overlapped(host, h00, mcs_now, mcs_per_step, args.e2e_slabs)
+            mcs_now += mcs_per_step
+        torch.cuda.synchronize()
+        overl = (n_e2e * att_per_step, time.perf_counter() - w0)
         if args.config == 3 or args.pipeline:
             # lane 1: a genuinely different lattice -- grown under another Philox key, then advanced (like lane 0) under
             # the handle's key; the lane clocks differ as well
@@ -241,12 +252,18 @@ def run_ours(args):
     except Exception as exc:   # e.g. not enough pinned host memory on the box
         e2e_err = str(exc)[:200]
     _, serial_s, serial_rate = shard.aggregate(serial[0], serial[1], device=dev)
+    _, overl_s, overl_rate = shard.aggregate(overl[0], overl[1], device=dev)
     _, piped_s, piped_rate = shard.aggregate(piped[0], piped[1], device=dev)
     e2e = {"value": None, "unit": UNIT,
            "h2d_bytes_per_step": k.lattice_bytes + 8 * R, "d2h_bytes_per_step": k.lattice_bytes + (3 * 8 + 32) * R}
     if serial_s != float("inf"):
         e2e.update({"value": serial_rate / 1e9, "steps": n_e2e,
                     "api": "kpz_step_host: ONE pinned host lattice copied in, advanced, measured and copied out per step"})
+    if overl_s != float("inf"):
+        e2e.update({"value": overl_rate / 1e9, "steps": n_e2e, "sequential_value": serial_rate / 1e9,
+                    "api": "kpz_step_host_overlapped (%d slabs): ONE pinned host lattice copied in, advanced, measured and "
+                           "copied out per step, the copies overlapped with the colour passes slab by slab; "
+                           "sequential_value = the same through kpz_step_host (copy, kernels, copy in sequence)" % args.e2e_slabs})
     if piped_s != float("inf"):
         e2e.update({"two_lane_value": piped_rate / 1e9, "two_lane_steps": 2 * n_rounds,
                     "two_lane_api": "kpz_pipeline_host: two independent pinned host lattices; the copies of step b-1 / "
@@ -528,6 +545,7 @@ def main():
     ap.add_argument("--L", type=int, default=0, help="override the lattice size (debugging only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--pipeline", action="store_true", help="also time kpz_pipeline_host for configs other than 3")
+    ap.add_argument("--e2e-slabs", type=int, default=8, help="row slabs of kpz_step_host_overlapped in the e2e leg")
     ap.add_argument("--peaks", action="store_true", help="print the pipe micro-benchmarks (kpz_measure_peaks) and exit")
     ap.add_argument("--slabs", action="store_true", help="ONE lattice of the config split into slabs of rows over the N ranks "
                                                          "(strong scaling; DESIGN.md Multi-GPU) instead of one lattice per rank")

@@ -200,6 +200,18 @@ int32_t kpz_import_packed(kpz_ctx* ctx, const void* host_src, size_t bytes, cons
 int32_t kpz_step_host(kpz_ctx* ctx, void* host_lattice, size_t bytes, int64_t* h00_inout, uint64_t mcs_start,
                       uint64_t mcs, int64_t* sum_h, int64_t* sum_h2, double* W2);
 
+/* kpz_step_host with the copies OVERLAPPED with the kernels for ONE lattice: the
+ * lattice travels in n_slabs blocks of rows; as soon as a block has arrived all `mcs` MCS run on the part of it that
+ * cannot depend on rows still in flight (dependencies spread by tile + 1 rows per colour pass), rows that are final are
+ * copied back while later blocks still compute, and the last stage completes the rest in pass order.  Same kernels,
+ * same results as kpz_step_host, bit for bit.  host_lattice should be pinned memory (pageable memory makes the copies
+ * synchronous: still correct, no overlap).  The n_slabs blocks ramp up in height (x2) from both ends of the lattice, so that
+ * only a short first copy-in and a short last copy-out are exposed.  Needs n_replicas = 1, the default schedule on the tiled
+ * kernel, n_slabs >= 2 and every block taller than 8 mcs (tile + 1) + 4 tile rows (n_slabs is reduced until that holds);
+ * otherwise it IS kpz_step_host.  Synchronises before returning. */
+int32_t kpz_step_host_overlapped(kpz_ctx* ctx, void* host_lattice, size_t bytes, int64_t* h00_inout, uint64_t mcs_start,
+                                 uint64_t mcs, uint32_t n_slabs, int64_t* sum_h, int64_t* sum_h2, double* W2);
+
 /* Pipelined end-to-end steps with HOST buffers: n_lanes independent lattices
  * (same L, p, q, tile, seed as the handle; they differ in state and MCS clock), each a HOST buffer of `bytes` >=
  * lattice_bytes in the device layout above (pinned memory is required for the copies to overlap), are each advanced

@@ -25,6 +25,7 @@ exported_symbols = [
     "kpz_set_path", "kpz_measure_peaks",
     "kpz_slab_workspace_bytes", "kpz_create_slab", "kpz_slab_info", "kpz_global_draw", "kpz_slab_pass", "kpz_slab_end_mcs",
     "kpz_slab_measure_local", "kpz_slab_measure_finish", "kpz_slab_finalize", "kpz_measure_static",
+    "kpz_step_host_overlapped",
 ]
 
 
@@ -84,6 +85,7 @@ def load_library() -> ctypes.CDLL:
         "kpz_slab_measure_finish": [vp, vp, vp, vp],
         "kpz_slab_finalize": [u32, vp, i64, vp, vp, vp],
         "kpz_measure_static": [vp, u32, vp],
+        "kpz_step_host_overlapped": [vp, vp, sz, vp, u64, u64, u32, vp, vp, vp],
     }
     for name, args in sig.items():
         fn = getattr(L, name)
@@ -275,6 +277,17 @@ class KPZ:
         w2 = np.zeros(R, dtype=np.float64)
         self._check(self._lib.kpz_step_host(self._h, host_tensor.data_ptr(), host_tensor.numel(), h00.ctypes.data,
                                             int(mcs_start), int(mcs), s1.ctypes.data, s2.ctypes.data, w2.ctypes.data))
+        return s1, s2, w2
+
+    def step_host_overlapped(self, host_tensor, h00, mcs_start, mcs, n_slabs=4):
+        """kpz_step_host_overlapped: kpz_step_host with the copies of ONE lattice overlapped with its kernels slab by slab."""
+        R = self.n_replicas
+        s1 = np.zeros(R, dtype=np.int64)
+        s2 = np.zeros(R, dtype=np.int64)
+        w2 = np.zeros(R, dtype=np.float64)
+        self._check(self._lib.kpz_step_host_overlapped(self._h, host_tensor.data_ptr(), host_tensor.numel(), h00.ctypes.data,
+                                                       int(mcs_start), int(mcs), int(n_slabs), s1.ctypes.data,
+                                                       s2.ctypes.data, w2.ctypes.data))
         return s1, s2, w2
 
     def pipeline_host(self, host_tensors, h00, mcs_start, mcs, n_rounds=1):

@@ -2,6 +2,7 @@
 // No CPU fallback: every entry point that computes launches CUDA kernels on the bound stream.
 #include "kpz_host.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstring>
 #include <new>
@@ -104,6 +105,8 @@ void fill_update_params(const kpz_ctx* c, kpz::UpdateParams& P, uint32_t m, uint
     P.HNy = slab ? P.NT / c->n_slabs / 2 : P.HN;
     P.ty0 = slab ? c->slab * (P.NT / c->n_slabs) : 0u;
     P.ywrap = slab ? 0xFFFFFFFFu : c->L;
+    P.j0 = 0u;
+    P.tywrap = slab ? 0xFFFFFFFFu : P.NT;
     if (slab) P.plane_words = (uint64_t)c->rows * (c->L / 32);
     P.tiles_per_colour = P.HN * P.HNy;
     P.total_items = (uint64_t)c->R * P.tiles_per_colour;
@@ -902,6 +905,155 @@ int32_t kpz_pipeline_host(kpz_ctx* c, void* device_lattice2, size_t device_latti
     }
     if (h00_inout) std::memcpy(h00_inout, h00.data(), h00.size() * sizeof(int64_t));
     return worst;
+}
+
+// ---- kpz_step_host_overlapped: one lattice, copies overlapped with the kernels slab by slab -------------------------
+// A colour pass of a tile touches only the T + 1 storage rows of its footprint, so dependencies between passes spread
+// by at most T + 1 rows per pass.  The lattice is cut into n_slabs blocks of rows that arrive one after the other.
+// After block s has arrived, stage s runs ALL P = 4 mcs passes, pass p on the tiles whose footprint lies inside
+//   [ g_p , f_{s,p} ],   g_p = p (T + 1),   f_{s,p} = (last arrived row) - p (T + 1),
+// (the blocks are small at both ends and large in the middle, see below)
+// and that no earlier stage has processed: every earlier-pass tile that meets such a footprint lies inside the region
+// of an earlier pass of a stage <= s, hence was launched before.  The last stage takes everything that is left (the
+// wedges below g_p and above the last frontier, including the tile row that wraps around the lattice edge), again in
+// pass order.  Rows that no later tile can touch are copied back while later stages still compute.  Same kernels, same
+// tile ids, same streams as kpz_run: the trajectory is bit-identical (tests/test_gpu_parity.py).
+namespace {
+
+inline long long floor_div(long long a, long long b) { return a >= 0 ? a / b : -((-a + b - 1) / b); }
+inline long long ceil_div(long long a, long long b) { return -floor_div(-a, b); }
+
+// launches colour pass `slot` of MCS m on the tile rows [a, b] (frame of MCS m; b may exceed NT - 1: wrapped range)
+int32_t launch_pass_rows(kpz_ctx* c, uint32_t m, uint32_t slot, uint32_t cy, long long a, long long b) {
+    if (b < a) return KPZ_OK;
+    const long long jf = a > (long long)cy ? (a - cy + 1) / 2 : 0;       // ceil((a - cy) / 2), >= 0
+    if (b < (long long)cy) return KPZ_OK;
+    const long long jl = (b - cy) / 2;
+    if (jl < jf) return KPZ_OK;
+    kpz::UpdateParams P;
+    fill_update_params(c, P, m, slot, 0u);
+    P.j0 = (uint32_t)jf;
+    P.HNy = (uint32_t)(jl - jf + 1);
+    P.tiles_per_colour = P.HN * P.HNy;
+    P.total_items = (uint64_t)P.tiles_per_colour;
+    P.blocked = (P.HN % 8 == 0 && P.HNy % 4 == 0) ? 1u : 0u;
+    return c->T >= 32 ? kpz_launch_update_wide(c, P) : kpz_launch_update_narrow(c, P);
+}
+
+}  // namespace
+
+int32_t kpz_step_host_overlapped(kpz_ctx* c, void* host_lattice, size_t bytes, int64_t* h00_inout, uint64_t mcs_start,
+                                 uint64_t mcs, uint32_t n_slabs, int64_t* sum_h, int64_t* sum_h2, double* W2) {
+    int32_t rc = require_bound(c);
+    if (rc != KPZ_OK) return rc;
+    DeviceGuard dg__(c->device);
+    if ((rc = require_whole(c)) != KPZ_OK) return rc;
+    if (!host_lattice || bytes < c->lattice_bytes || mcs_start + mcs > 0xFFFFFFFFull) return kpz_fail(c, KPZ_EINVAL, "bad argument");
+    const long long L = c->L, T = c->T, NT = L / T, P_ = 4 * (long long)mcs, step = T + 1;
+    ResidentPlan pl{};
+    // the overlap needs: one replica, the default schedule on the tiled kernel, and slabs much taller than the
+    // region the P passes eat away on both sides; otherwise the plain sequence (same result)
+    // Slab heights: compute is the bottleneck (the kernels of a step take about three times its copies), so only the
+    // FIRST copy-in and the LAST copy-out are exposed: the slabs ramp up geometrically (x2) from both ends and are
+    // large in the middle (few launches, little tail).  Every slab must be taller than C_min.
+    const long long C_min = 2 * P_ * step + 4 * T;
+    std::vector<long long> B;                                               // row boundaries B[0] = 0 .. B[S] = L
+    bool eligible = c->R == 1 && c->schedule == KPZ_SCHEDULE_COLOURS && c->sub_sweeps == 1 && !c->poisson && mcs >= 1 &&
+                    n_slabs >= 2 && choose_path(c, pl) == KPZ_PATH_TILED;
+    if (eligible) {
+        eligible = false;
+        for (long long S_try = n_slabs; S_try >= 2 && !eligible; --S_try) {
+            std::vector<long long> w((size_t)S_try);
+            long long wsum = 0;
+            for (long long i = 0; i < S_try; ++i) {
+                const long long e = std::min(i, S_try - 1 - i);
+                w[(size_t)i] = 1ll << std::min<long long>(e, 20);
+                wsum += w[(size_t)i];
+            }
+            B.assign(1, 0);
+            long long acc = 0;
+            bool ok = true;
+            for (long long i = 0; i < S_try; ++i) {
+                acc += w[(size_t)i];
+                const long long b = (i == S_try - 1) ? L : (L * acc / wsum) / (2 * T) * (2 * T);     // whole tile-row pairs
+                if (b - B.back() < C_min) { ok = false; break; }
+                B.push_back(b);
+            }
+            eligible = ok;
+        }
+    }
+    if (!eligible) return kpz_step_host(c, host_lattice, bytes, h00_inout, mcs_start, mcs, sum_h, sum_h2, W2);
+    const long long S = (long long)B.size() - 1;
+    const size_t row_bytes = (size_t)L / 8, plane_bytes = (size_t)L * row_bytes;
+    unsigned char* hb = static_cast<unsigned char*>(host_lattice);
+    unsigned char* db = reinterpret_cast<unsigned char*>(c->d_lattice);
+    // bookkeeping copies first, while the copy engines are idle
+    if ((rc = set_h00(c, h00_inout)) != KPZ_OK) return rc;
+    if ((rc = pipeline_resources(c, (size_t)(2 * S + 2))) != KPZ_OK) return rc;
+    cudaEvent_t* ev_in = c->events.data();
+    cudaEvent_t* ev_cmp = c->events.data() + S;
+    c->mcs = mcs_start;
+    c->attempts_base = mcs_start * (uint64_t)c->L * c->L;
+    // all slabs are queued on the copy-in stream at once: they arrive in order
+    for (long long s = 0; s < S; ++s) {
+        for (int pln = 0; pln < 2; ++pln) {
+            const size_t off = pln * plane_bytes + (size_t)B[(size_t)s] * row_bytes;
+            KPZ_CUDA(c, cudaMemcpyAsync(db + off, hb + off, (size_t)(B[(size_t)s + 1] - B[(size_t)s]) * row_bytes,
+                                        cudaMemcpyHostToDevice, c->s_in));
+        }
+        KPZ_CUDA(c, cudaEventRecord(ev_in[s], c->s_in));
+    }
+    auto copy_out_rows = [&](long long r0, long long r1) -> int32_t {      // rows [r0, r1] of both planes
+        if (r1 < r0) return KPZ_OK;
+        for (int pln = 0; pln < 2; ++pln) {
+            const size_t off = pln * plane_bytes + (size_t)r0 * row_bytes;
+            KPZ_CUDA(c, cudaMemcpyAsync(hb + off, db + off, (size_t)(r1 - r0 + 1) * row_bytes, cudaMemcpyDeviceToHost, c->s_out));
+        }
+        return KPZ_OK;
+    };
+    const long long g_last = (P_ - 1) * step;                               // g_{P-1}
+    long long out_next = g_last + T;                                        // first row not yet copied back
+    for (long long s = 0; s < S; ++s) {
+        KPZ_CUDA(c, cudaStreamWaitEvent(c->stream, ev_in[s], 0));
+        for (long long p = 0; p < P_; ++p) {
+            const uint32_t m = (uint32_t)(mcs_start + (uint64_t)(p / 4)), slot = (uint32_t)(p % 4);
+            uint32_t ox, oy, perm[4];
+            host_global_draw(c, m, 0u, 0u, &ox, &oy, perm);
+            const uint32_t cy = perm[slot] >> 1;
+            const long long g = p * step;
+            const long long t_lo = ceil_div(g - (long long)oy, T) < 0 ? 0 : ceil_div(g - (long long)oy, T);
+            auto t_hi = [&](long long stage) { return floor_div((B[(size_t)stage + 1] - 1 - p * step) - T - (long long)oy, T); };
+            long long a, b;
+            if (s < S - 1) {
+                a = s == 0 ? t_lo : std::max(t_lo, t_hi(s - 1) + 1);
+                b = t_hi(s);
+            } else {
+                a = std::max(t_lo, t_hi(S - 2) + 1);
+                b = NT - 1 + t_lo;                                          // wraps: tile rows 0 .. t_lo - 1 come last
+            }
+            if ((rc = launch_pass_rows(c, m, slot, cy, a, b)) != KPZ_OK) return rc;
+        }
+        KPZ_CUDA(c, cudaEventRecord(ev_cmp[s], c->stream));
+        KPZ_CUDA(c, cudaStreamWaitEvent(c->s_out, ev_cmp[s], 0));
+        if (s < S - 1) {
+            const long long hi = (B[(size_t)s + 1] - 1 - (P_ - 1) * step) - T;  // rows <= f_{s,P-1} - T are final
+            if ((rc = copy_out_rows(out_next, hi)) != KPZ_OK) return rc;
+            if (hi >= out_next) out_next = hi + 1;
+        } else {
+            if ((rc = copy_out_rows(out_next, L - 1)) != KPZ_OK) return rc;
+            if ((rc = copy_out_rows(0, g_last + T - 1)) != KPZ_OK) return rc;
+        }
+    }
+    c->mcs = mcs_start + mcs;
+    c->attempts_base = c->mcs * (uint64_t)c->L * c->L;
+    rc = kpz_measure(c, sum_h, sum_h2, W2);                                 // reads the final lattice while it is copied back
+    if (rc != KPZ_OK && rc != KPZ_EOVERFLOW) { cudaStreamSynchronize(c->s_out); return rc; }
+    if (h00_inout) {
+        const int32_t r2 = get_h00(c, h00_inout);
+        if (r2 != KPZ_OK) { cudaStreamSynchronize(c->s_out); return r2; }
+    }
+    KPZ_CUDA(c, cudaStreamSynchronize(c->s_out));
+    return rc;
 }
 
 // profiles of replica `replica` relative to h00 on the device (scratch prof[2][L]) + spectra; shared by the two calls

@@ -67,6 +67,10 @@ struct UpdateParams {
     uint32_t HNy;                  // tile rows of one colour in this launch
     uint32_t ty0;                  // first global tile row of the stored rows
     uint32_t ywrap;                // row index at which the stored rows wrap around: L, or 0xFFFFFFFF for a slab (never)
+    // A launch may cover only the tile-row pairs j0 .. j0 + HNy - 1 of a whole lattice (kpz_step_host_overlapped runs the
+    // colour passes slab by slab while the rest of the lattice is still in flight); a tile row index >= tywrap wraps.
+    uint32_t j0;                   // first tile-row pair of this launch (0: from the first)
+    uint32_t tywrap;               // NT for a whole lattice, 0xFFFFFFFF for a slab
     uint32_t blocked;              // 1: 8x4 lane blocking of tiles (HN % 8 == 0), 0: linear
     uint32_t m;                    // MCS index (number of completed MCS)
     uint32_t slot;                 // 0..3: which entry of the colour order this launch executes
@@ -685,7 +689,9 @@ __global__ void __launch_bounds__(NTHR, (T == 64) ? 3 : (T == 32 ? 8 : 1)) kpz_u
     }
     uint32_t ox, oy, colour;
     global_draw<T>(P, SUB ? P.sub : 0u, replica, ox, oy, colour);
-    const uint32_t tx = DEAD ? i : 2u * i + (colour & 1u), tyl = DEAD ? j : 2u * j + (colour >> 1);
+    const uint32_t tx = DEAD ? i : 2u * i + (colour & 1u);
+    uint32_t tyl = DEAD ? j : 2u * (j + P.j0) + (colour >> 1);
+    if (tyl >= P.tywrap) tyl -= P.tywrap;                     // a launch over a wrapped range of tile rows
     const uint32_t ty = tyl + P.ty0;                          // global tile row (tyl: within the stored rows)
     const uint32_t X0 = ox + tx * T, Y0 = oy + tyl * T;       // < L + T
     const uint32_t tile_id = ty * P.NT + tx;

@@ -385,6 +385,64 @@ def test_run_split_checkpoint_and_step_host(pkg):
     assert torch.equal(host, host2)                 # step_host wrote the advanced lattice back
 
 
+@pytest.mark.parametrize("L,T,p,q,S,mcs,seed", [
+    (2048, 16, 1.0, 0.0, 4, 3, 95),            # 4 slabs of 512 rows, 12 passes eat 204 rows per side
+    (2048, 16, 0.75, 0.25, 2, 5, 96),
+    (4096, 32, 1.0, 0.0, 4, 2, 97),
+    (4096, 32, 0.6, 0.2, 8, 1, 98),            # slabs of 512 rows: just tall enough for 4 passes of T = 32
+    (8192, 64, 1.0, 0.0, 4, 2, 99),
+    (8192, 64, 0.75, 0.25, 2, 3, 100),
+    (6144, 64, 1.0, 0.0, 3, 2, 101),           # L not a power of two, three slabs
+])
+def test_step_host_overlapped_matches_oracle_and_plain_step(pkg, L, T, p, q, S, mcs, seed):
+    """kpz_step_host_overlapped: one lattice through pinned HOST memory with its copies overlapped slab by slab with the
+    colour passes (a trapezoid of passes per slab, the wedges last).  Three steps in a row from the flat state: sums,
+    W^2, h(0,0), counters and the host lattice itself against the oracle and against kpz_step_host."""
+    import torch
+    a = pkg.KPZ(L, p, q, T, seed)
+    b = pkg.KPZ(L, p, q, T, seed)
+    a.set_path("tiled"); b.set_path("tiled")
+    a.init_flat()
+    ha = torch.empty(a.lattice_bytes, dtype=torch.uint8).pin_memory()
+    a.export_packed(ha)
+    hb = ha.clone().pin_memory()
+    h00a, h00b = np.zeros(1, dtype=np.int64), np.zeros(1, dtype=np.int64)
+    o = Oracle(L, p, q, T, seed, threads=NTHREADS)
+    o.init_flat()
+    t = 0
+    for step in range(3):
+        l0 = a.launch_count()
+        ra = a.step_host_overlapped(ha, h00a, t, mcs, S)
+        assert a.launch_count() - l0 > 4 * mcs + 3          # the passes were really split over the slabs
+        rb = b.step_host(hb, h00b, t, mcs)
+        o.run(mcs)
+        t += mcs
+        want = o.measure()
+        assert (int(ra[0][0]), int(ra[1][0]), float(ra[2][0])) == want == (int(rb[0][0]), int(rb[1][0]), float(rb[2][0]))
+        assert int(h00a[0]) == int(h00b[0]) == o.counters()["h00"]
+        assert torch.equal(ha, hb), "host lattices differ after step %d" % step
+        assert a.state_hash() == o.state_hash()
+        ca, oc = a.counters(), o.counters()
+        assert (ca["deposits"], ca["removals"], ca["mcs"], ca["attempts"]) == (oc["deposits"], oc["removals"], oc["mcs"], oc["attempts"])
+
+
+def test_step_host_overlapped_falls_back_when_it_cannot_overlap(pkg):
+    """Too many passes for the slab height, several replicas, a resident-path lattice: the call IS kpz_step_host."""
+    import torch
+    for (L, T, R, S, mcs) in ((2048, 64, 1, 8, 4), (256, 16, 3, 2, 2), (128, 16, 1, 2, 1)):
+        k = pkg.KPZ(L, 0.75, 0.25, T, 31, n_replicas=R)
+        k.init_flat()
+        host = torch.empty(k.lattice_bytes, dtype=torch.uint8).pin_memory()
+        k.export_packed(host)
+        h00 = np.zeros(R, dtype=np.int64)
+        s1, s2, w2 = k.step_host_overlapped(host, h00, 0, mcs, S)
+        for r in range(R):
+            o = Oracle(L, 0.75, 0.25, T, 31, replica=r, threads=NTHREADS)
+            o.init_flat(); o.run(mcs)
+            assert (int(s1[r]), int(s2[r]), float(w2[r])) == o.measure() and int(h00[r]) == o.counters()["h00"]
+            assert k.state_hash(r) == o.state_hash()
+
+
 def _host_ram_gib():
     for line in open("/proc/meminfo"):
         if line.startswith("MemAvailable:"):
