@@ -547,6 +547,7 @@ def main():
     ap.add_argument("--pipeline", action="store_true", help="also time kpz_pipeline_host for configs other than 3")
     ap.add_argument("--e2e-slabs", type=int, default=8, help="row slabs of kpz_step_host_overlapped in the e2e leg")
     ap.add_argument("--peaks", action="store_true", help="print the pipe micro-benchmarks (kpz_measure_peaks) and exit")
+    ap.add_argument("--layouts", action="store_true", help="print the tile-layout experiment (kpz_measure_layouts) and exit")
     ap.add_argument("--slabs", action="store_true", help="ONE lattice of the config split into slabs of rows over the N ranks "
                                                          "(strong scaling; DESIGN.md Multi-GPU) instead of one lattice per rank")
     ap.add_argument("--launcher-selftest", action="store_true", help="multi-rank launch + reductions only (gloo, no GPU)")
@@ -567,6 +568,11 @@ def main():
     if args.peaks:
         import paper_1110_6745_b200 as pkg
         print(json.dumps({"peaks": pkg.measure_peaks(), "units": "per second; see include/kpz.h kpz_measure_peaks"}))
+        return
+    if args.layouts:
+        import paper_1110_6745_b200 as pkg
+        print(json.dumps({"layouts": pkg.measure_layouts(), "units": "attempts/s of the T = 64 attempt loop alone, resident warps "
+                          "per SM; see include/kpz.h kpz_measure_layouts"}))
         return
     run_ours(args)
 

@@ -311,6 +311,18 @@ int32_t kpz_launch_count(const kpz_ctx* ctx, uint64_t* out);
 #define KPZ_N_PEAKS 11
 int32_t kpz_measure_peaks(double* out, uint32_t n);
 
+/* Tile-layout experiment behind DESIGN.md section 7.1 ("fewer words per tile"): runs, on the CURRENT device, the attempt
+ * loop of the T = 64, p = 1, q = 0 kernel ALONE (4096 attempts per tile on tiles of random bits, no staging, nothing
+ * written back) in two shared-memory layouts and writes KPZ_N_LAYOUTS doubles to the HOST array `out`:
+ *   [0] attempts/s, [1] resident warps per SM: the update kernel's own layout and code (three words per row, 199 words
+ *       per tile) -- the ceiling of the present kernel without its staging;
+ *   [2] attempts/s, [3] resident warps per SM: tile and halo as one bit string with a row pitch of 66 bits (138 words
+ *       per tile): no halo words, but the rows above and below need a rotate each and their own word index.
+ * A measurement of a design alternative, not a step of the path.  KPZ_EINVAL for a NULL / short array, KPZ_ECUDA
+ * without a device. */
+#define KPZ_N_LAYOUTS 4
+int32_t kpz_measure_layouts(double* out, uint32_t n);
+
 /* Device Philox4x32-10 self-test: evaluates n (counter,key) inputs on the GPU.  HOST arrays: ctr[4n], key[2n],
  * out[4n].  Used by the tests to check the in-kernel generator against the published known answers. */
 int32_t kpz_philox_selftest(const uint32_t* ctr, const uint32_t* key, uint32_t* out, uint32_t n);

@@ -22,7 +22,7 @@ exported_symbols = [
     "kpz_destroy", "kpz_synchronize", "kpz_last_error", "kpz_get_slopes", "kpz_get_window", "kpz_set_slopes",
     "kpz_state_hash", "kpz_counters", "kpz_export_packed", "kpz_import_packed", "kpz_step_host", "kpz_pipeline_host",
     "kpz_launch_count", "kpz_philox_selftest", "kpz_profiles", "kpz_power_spectrum", "kpz_set_schedule", "kpz_set_sub_sweeps", "kpz_run_sampled", "kpz_set_poisson",
-    "kpz_set_path", "kpz_measure_peaks",
+    "kpz_set_path", "kpz_measure_peaks", "kpz_measure_layouts",
     "kpz_slab_workspace_bytes", "kpz_create_slab", "kpz_slab_info", "kpz_global_draw", "kpz_slab_pass", "kpz_slab_end_mcs",
     "kpz_slab_measure_local", "kpz_slab_measure_finish", "kpz_slab_finalize", "kpz_measure_static",
     "kpz_step_host_overlapped",
@@ -75,6 +75,7 @@ def load_library() -> ctypes.CDLL:
         "kpz_launch_count": [vp, vp],
         "kpz_philox_selftest": [vp, vp, vp, u32],
         "kpz_measure_peaks": [vp, u32],
+        "kpz_measure_layouts": [vp, u32],
         "kpz_slab_workspace_bytes": [u32, u32, u32, vp, vp],
         "kpz_create_slab": [vp, u32, dbl, dbl, u32, u64, u32, u32],
         "kpz_slab_info": [vp, vp, vp, vp, vp, vp],
@@ -116,6 +117,18 @@ def measure_peaks():
     if rc != KPZ_OK:
         raise KpzError(rc, "kpz_measure_peaks")
     return dict(zip(PEAK_NAMES, out.tolist()))
+
+
+LAYOUT_NAMES = ("rows3_attempts_per_s", "rows3_warps_per_sm", "pitch66_attempts_per_s", "pitch66_warps_per_sm")
+
+
+def measure_layouts():
+    """kpz_measure_layouts on the current device -> dict (the attempt loop alone in two tile layouts, include/kpz.h)."""
+    out = np.zeros(len(LAYOUT_NAMES), dtype=np.float64)
+    rc = load_library().kpz_measure_layouts(out.ctypes.data, len(out))
+    if rc != KPZ_OK:
+        raise KpzError(rc, "kpz_measure_layouts")
+    return dict(zip(LAYOUT_NAMES, out.tolist()))
 
 
 def philox_selftest(ctr, key):

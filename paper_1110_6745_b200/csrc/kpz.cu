@@ -316,6 +316,42 @@ cudaError_t run_peak(uint32_t blocks, uint32_t iters, uint32_t* sink, unsigned l
     return e;
 }
 
+// the attempt loop of T = 64 alone in tile layout LAYOUT (kpz_peaks.cuh): attempts/s with `waves` CTAs per CTA slot
+template <int LAYOUT>
+cudaError_t run_layout(int sms, uint32_t* sink, double* attempts_per_s, double* warps_per_sm) {
+    constexpr int NTHR = 96;
+    const size_t smem = (size_t)(LAYOUT ? kpz::LAYOUT66_WORDS : kpz::TileGeom<64>::WORDS) * NTHR * sizeof(uint32_t);
+    cudaError_t e = cudaFuncSetAttribute(kpz::kpz_layout_kernel<LAYOUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kpz::kpz_layout_kernel<LAYOUT>, NTHR, smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm <= 0) return cudaErrorInvalidConfiguration;
+    *warps_per_sm = per_sm * (NTHR / 32.0);
+    const uint32_t blocks = (uint32_t)(sms * per_sm * 8);        // eight full waves
+    cudaEvent_t e0, e1;
+    e = cudaEventCreate(&e0);
+    if (e != cudaSuccess) return e;
+    e = cudaEventCreate(&e1);
+    if (e != cudaSuccess) { cudaEventDestroy(e0); return e; }
+    kpz::kpz_layout_kernel<LAYOUT><<<blocks, NTHR, smem>>>(0x9E3779B9u, 1u, 2u, 1u << 27, sink);      // warm-up
+    float best = 1e30f;
+    for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {
+        cudaEventRecord(e0);
+        kpz::kpz_layout_kernel<LAYOUT><<<blocks, NTHR, smem>>>(0x9E3779B9u + rep, 2u + rep, 2u, 1u << 27, sink);
+        cudaEventRecord(e1);
+        e = cudaEventSynchronize(e1);
+        float t = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&t, e0, e1);
+        if (e == cudaSuccess && t < best) best = t;
+    }
+    if (e == cudaSuccess) e = cudaGetLastError();
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    *attempts_per_s = (double)blocks * NTHR * 4096.0 / (best * 1e-3);
+    return e;
+}
+
 // ---- kpz_measure_static: the measurement with its scratch in a file-scope static array (no allocation) ----------
 // For callers that cannot allocate (code under CUDA graph capture, tight serving loops).  The partial sums of the
 // measurement kernels -- row-0 prefix, per-chunk (S0, S1, S2) of every column, the four 64-bit half-accumulators --
@@ -1308,6 +1344,20 @@ int32_t kpz_measure_peaks(double* out, uint32_t n) {
     out[6] = lanes / (ms[5] * 1e-3);                   // shared-memory XOR reductions (lane-ops/s)
     out[7] = lanes / 4.0 / (ms[6] * 1e-3);             // attempts/s of the bare instruction mix of one p = 1 attempt, no chain
     out[8] = (double)sms;
+    return KPZ_OK;
+}
+
+int32_t kpz_measure_layouts(double* out, uint32_t n) {
+    if (!out || n < KPZ_N_LAYOUTS) return KPZ_EINVAL;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return KPZ_ECUDA;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) return KPZ_ECUDA;
+    uint32_t* sink = nullptr;
+    if (cudaMalloc(&sink, sizeof(uint32_t)) != cudaSuccess) { cudaGetLastError(); return KPZ_ECUDA; }
+    cudaError_t e = run_layout<0>(sms, sink, &out[0], &out[1]);
+    if (e == cudaSuccess) e = run_layout<1>(sms, sink, &out[2], &out[3]);
+    cudaFree(sink);
+    if (e != cudaSuccess) { cudaGetLastError(); return KPZ_ECUDA; }
     return KPZ_OK;
 }
 

@@ -10,6 +10,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "kpz_device.cuh"
+
 namespace kpz {
 
 enum PeakKind { PEAK_LOP3 = 0, PEAK_SHF = 1, PEAK_IMAD = 2, PEAK_IMAD_WIDE = 3, PEAK_LDS = 4, PEAK_ATOMS = 5, PEAK_MIX = 6 };
@@ -109,6 +111,83 @@ __global__ void __launch_bounds__(512) kpz_chain_kernel(uint32_t iters, uint32_t
     }
     const long long t1 = clock64();
     if (threadIdx.x == 0) ticks[0] = (unsigned long long)(t1 - t0);
+}
+
+
+// ---- the attempt loop alone, in two tile layouts (fewer words per tile) -------------------
+// Shared memory decides the occupancy of the T = 64 kernel: 199 words per tile = 9 warps per SM.  LAYOUT 0 runs the
+// update kernel's own attempt loop (run_tile_steps, MODE 0) on a tile of random bits without the staging -- the ceiling of
+// the present layout.  LAYOUT 1 is the cheapest layout with fewer words that was found: the 66 x 66 bits of tile and halo as
+// ONE bit string with a row pitch of 66 bits (138 words = 12 warps per SM).  Left / right neighbours then need no halo word
+// (the funnel shifts cross the row ends by themselves), but the rows above and below sit 2 bits off and need a rotate
+// each, and three word indices instead of one.  Same Philox calls, same five loads, tests and XOR reduction; what is
+// measured is whether three more warps per SM pay for the two rotates and the address arithmetic.  NOT a kernel of the
+// path: the tile holds random bits and nothing is written back.
+constexpr int LAYOUT66_WORDS = 138;
+
+template <int NTHR>
+__device__ __forceinline__ void attempt_pitch66(uint32_t* __restrict__ sm, uint32_t site_word, float& dep_f, uint32_t two,
+                                                uint32_t two27) {
+    const uint32_t idx = site_word >> 20, ly = site_word >> 26;
+    // q = ly * 66 + lx: bit position of the site in the string, + 96.  The multiplier pipe is the idle one: q by IMAD, the
+    // word indices of the rows above / below as the high halves of q * 2^27 + c * 2^27 (IMAD.WIDE) instead of add + shift
+    // (the multipliers 2 and 2^27 arrive as kernel arguments: ptxas turns constant powers of two back into shifts and adds)
+    uint32_t q;
+    asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(q) : "r"(ly), "r"(two), "r"(idx));
+    unsigned long long pu, pd;
+    asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(pu) : "r"(q), "r"(two27), "l"(162ull << 27));
+    asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(pd) : "r"(q), "r"(two27), "l"(30ull << 27));
+    uint32_t* a = sm + ((q >> 5) + 3u) * NTHR;
+    const uint32_t wo = a[0], wp = *(a - NTHR), wn = a[NTHR];
+    const uint32_t wu = sm[(uint32_t)(pu >> 32) * NTHR];    // bit (q + 2) & 31 of the word that holds position + 66
+    const uint32_t wd = sm[(uint32_t)(pd >> 32) * NTHR];    // bit (q - 2) & 31 of the word that holds position - 66
+    const uint32_t wl = __funnelshift_l(wp, wo, 1), wr = __funnelshift_r(wo, wn, 1);
+    const uint32_t wua = __funnelshift_r(wu, wu, 2), wda = __funnelshift_l(wd, wd, 2);
+    const uint32_t bit = __funnelshift_l(0u, 1u, q);
+    const uint32_t t1 = lop3<0xDB>(wo, wl, wr), t2 = lop3<0xBD>(wo, wua, wda);
+    const uint32_t md0 = lop3_and_not_not(bit, t1, t2);
+    atomicXor(a, md0);
+    asm("{ .reg .pred p; setp.ne.u32 p, %1, 0; @p add.f32 %0, %0, 0f3F800000; }" : "+f"(dep_f) : "r"(md0));
+}
+
+template <int LAYOUT>
+__global__ void __launch_bounds__(96, LAYOUT ? 4 : 3) kpz_layout_kernel(uint32_t seed, uint32_t m, uint32_t two, uint32_t two27,
+                                                                             uint32_t* __restrict__ sink) {
+    constexpr int NTHR = 96;
+    constexpr int WORDS = LAYOUT ? LAYOUT66_WORDS : TileGeom<64>::WORDS;
+    extern __shared__ uint32_t smem[];
+    uint32_t* sm = smem + threadIdx.x;
+    const uint32_t tile_id = blockIdx.x * NTHR + threadIdx.x;
+    for (int w = 0; w < WORDS; ++w) sm[w * NTHR] = (tile_id * 2654435761u + (uint32_t)w * 0x9E3779B9u) ^ seed;
+    UpdateParams P = {};
+    P.key.k0 = seed;
+    P.key.k1 = ~seed;
+    P.m = m;
+    uint32_t n_dep = 0, n_rem = 0;
+    int32_t dh00 = 0;
+    if (LAYOUT == 0) {
+        run_tile_steps<64, NTHR, 0, false, false, 0>(sm, P, tile_id, 0u, n_dep, n_rem, dh00, 0xFFFFFFFFu, 0u);
+    } else {
+        float dep_f = 0.0f;
+        uint4 cur = philox4x32_10(0u, tile_id, P.m, 0u, P.key), nxt;
+#pragma unroll 4
+        for (uint32_t c = 0; c < 512u; ++c) {
+            nxt = philox4x32_10(c + 1u, tile_id, P.m, 0u, P.key);
+            attempt_pitch66<NTHR>(sm, cur.x, dep_f, two, two27);
+            attempt_pitch66<NTHR>(sm, cur.x * 4096u, dep_f, two, two27);
+            attempt_pitch66<NTHR>(sm, cur.y, dep_f, two, two27);
+            attempt_pitch66<NTHR>(sm, cur.y * 4096u, dep_f, two, two27);
+            attempt_pitch66<NTHR>(sm, cur.z, dep_f, two, two27);
+            attempt_pitch66<NTHR>(sm, cur.z * 4096u, dep_f, two, two27);
+            attempt_pitch66<NTHR>(sm, cur.w, dep_f, two, two27);
+            attempt_pitch66<NTHR>(sm, cur.w * 4096u, dep_f, two, two27);
+            cur = nxt;
+        }
+        n_dep = (uint32_t)dep_f;
+    }
+    uint32_t acc = n_dep;
+    for (int w = 0; w < WORDS; ++w) acc ^= sm[w * NTHR];
+    if (acc == 0x12345678u) sink[0] = acc;       // keeps the tile alive, practically never true
 }
 
 }  // namespace kpz

@@ -1072,3 +1072,25 @@ def test_dist_slab_single_rank_matches_oracle(pkg):
         d.h.close()
     finally:
         dist.destroy_process_group()
+
+
+def test_pipe_peaks_and_layout_measurements_are_physical(pkg):
+    """kpz_measure_peaks / kpz_measure_layouts (the figures the roofline and DESIGN.md section 7.1 quote) against what the
+    hardware fixes: no integer pipe issues more than 16 lanes per scheduler and clock, a bank-conflict-free warp load
+    moves at most 128 bytes per SM and clock, the dependent chain of a tile cannot beat the shared-memory latency, and the
+    occupancies of the two tile layouts are the ones their shared-memory footprints give on a 228 KB SM."""
+    pk = pkg.measure_peaks()
+    sms, clk = pk["n_sms"], pk["sm_clock_hz"]
+    assert sms >= 1 and 0.5e9 < clk < 4e9
+    lane_cap = sms * 4 * 16 * clk
+    for name in ("lop3_lane_ops", "shf_lane_ops", "imad_lane_ops"):
+        assert 0.5 * lane_cap < pk[name] < 1.05 * lane_cap, (name, pk[name], lane_cap)
+    assert pk["imad_wide_lane_ops"] < 0.6 * lane_cap
+    assert 0.5 * sms * 128 * clk < pk["lds_bytes"] < 1.05 * sms * 128 * clk
+    assert pk["attempt_mix"] * 5 * 4 * 32 / 32 <= 1.05 * pk["lds_bytes"]        # five 4-byte loads per attempt and lane
+    assert 20 < pk["chain_cycles_w1"] < pk["chain_cycles_w2"] < 2 * pk["chain_cycles_w1"]
+    ly = pkg.measure_layouts()
+    assert ly["rows3_warps_per_sm"] == 9 and ly["pitch66_warps_per_sm"] == 12
+    # an attempt of the present layout needs >= 9 ALU-pipe instructions + 2.4 of its share of a Philox call
+    assert 0 < ly["rows3_attempts_per_s"] < lane_cap / 11.0
+    assert 0 < ly["pitch66_attempts_per_s"] < lane_cap / 11.0
