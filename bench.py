@@ -59,7 +59,7 @@ ALG_BYTES_PER_UPDATE = 0.5            # HBM: each site (2 bits) read once and wr
 ALG_BYTES_PER_SITE_MEASURE = 0.125    # kpz_measure reads plane Y once (one bit per site)
 # dram__bytes_read.sum + dram__bytes_write.sum of one update launch at L = 2^17 (ncu --set full)
 TRAFFIC_BYTES_PER_LAUNCH = 6.26e9
-TRAFFIC_SOURCE = "profiles/r01_v9.md (ncu --set full, launch 46: 4.161 GB read + 2.103 GB written; kernel unchanged since)"
+TRAFFIC_SOURCE = "profiles/r02_ncu_full.md (ncu --set full on the final tree of round 2, launch 48: 4.154 GB read + 2.104 GB written)"
 
 
 def _peaks():
