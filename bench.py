@@ -150,6 +150,9 @@ def run_ours(args):
     cfg = dict(CONFIGS[args.config])
     if args.L:
         cfg["L"] = args.L
+    if args.tile:
+        cfg["tile"] = args.tile
+        cfg["name"] += " [tile overridden: %d]" % args.tile
     L, T, R, mcs_per_step = cfg["L"], cfg["tile"], cfg["replicas"], cfg["mcs_per_step"]
     general = not (cfg["p"] >= 1.0 and cfg["q"] <= 0.0)
     # weak scaling: every rank advances its own independent lattice(s) (its own Philox key)
@@ -543,6 +546,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, choices=sorted(CONFIGS), help="BASELINE config to time (default 3)")
     ap.add_argument("--L", type=int, default=0, help="override the lattice size (debugging only)")
+    ap.add_argument("--tile", type=int, default=0, help="override the tile edge (config 4 does not fix it: --config 4 --tile 8 "
+                                                        "runs the paper's own 8 x 8 cells)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--pipeline", action="store_true", help="also time kpz_pipeline_host for configs other than 3")
     ap.add_argument("--e2e-slabs", type=int, default=8, help="row slabs of kpz_step_host_overlapped in the e2e leg")
