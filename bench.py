@@ -197,9 +197,11 @@ def run_ours(args):
     value = rate / 1e9
 
     # ---- end to end through the C ABI with HOST buffers, copies inside the timed region ----
-    # "value": ONE pinned host lattice through kpz_step_host (H2D, kpz_run, kpz_measure, D2H in sequence: with one
-    # lattice a step's output is the next step's input, nothing can overlap).  "two_lane_value": two INDEPENDENT pinned
-    # host lattices through kpz_pipeline_host, the copies of one overlapping the kernels of the other.
+    # "value": ONE pinned host lattice through kpz_step_host_overlapped (a step's output is the next step's input, so steps
+    # cannot overlap, but the copies of a step overlap its own colour passes slab by slab: DESIGN.md 8.2);
+    # "sequential_value": the same through kpz_step_host (H2D, kpz_run, kpz_measure, D2H in sequence).
+    # "two_lane_value": two INDEPENDENT pinned host lattices through kpz_pipeline_host, the copies of one overlapping the
+    # kernels of the other.
     # Local timings first; the reductions over ranks come after the try block, so that a rank whose pinned
     # allocation fails still takes part in them (a leg that failed on any rank is reported as unavailable).
     serial = (0.0, float("inf"))
