@@ -22,7 +22,7 @@ exported_symbols = [
     "kpz_destroy", "kpz_synchronize", "kpz_last_error", "kpz_get_slopes", "kpz_get_window", "kpz_set_slopes",
     "kpz_state_hash", "kpz_counters", "kpz_export_packed", "kpz_import_packed", "kpz_step_host", "kpz_pipeline_host",
     "kpz_launch_count", "kpz_philox_selftest", "kpz_profiles", "kpz_power_spectrum", "kpz_set_schedule", "kpz_set_sub_sweeps", "kpz_run_sampled", "kpz_set_poisson",
-    "kpz_set_path", "kpz_measure_peaks", "kpz_measure_layouts",
+    "kpz_set_path", "kpz_measure_peaks", "kpz_measure_layouts", "kpz_overlap_plan",
     "kpz_slab_workspace_bytes", "kpz_create_slab", "kpz_slab_info", "kpz_global_draw", "kpz_slab_pass", "kpz_slab_end_mcs",
     "kpz_slab_measure_local", "kpz_slab_measure_finish", "kpz_slab_finalize", "kpz_measure_static",
     "kpz_step_host_overlapped",
@@ -76,6 +76,7 @@ def load_library() -> ctypes.CDLL:
         "kpz_philox_selftest": [vp, vp, vp, u32],
         "kpz_measure_peaks": [vp, u32],
         "kpz_measure_layouts": [vp, u32],
+        "kpz_overlap_plan": [u32, u32, u64, u32, vp, vp, vp, vp, vp, vp, vp],
         "kpz_slab_workspace_bytes": [u32, u32, u32, vp, vp],
         "kpz_create_slab": [vp, u32, dbl, dbl, u32, u64, u32, u32],
         "kpz_slab_info": [vp, vp, vp, vp, vp, vp],
@@ -117,6 +118,25 @@ def measure_peaks():
     if rc != KPZ_OK:
         raise KpzError(rc, "kpz_measure_peaks")
     return dict(zip(PEAK_NAMES, out.tolist()))
+
+
+def overlap_plan(L, tile, oy, n_slabs):
+    """kpz_overlap_plan (host only): the schedule of kpz_step_host_overlapped for a step of len(oy) MCS with y offsets oy.
+    -> (boundaries, launches[n][4] = stage, pass, first, last tile row, copies[n][3] = stage, first, last row), or None
+    when the shape does not allow the overlap."""
+    oy = np.ascontiguousarray(oy, dtype=np.uint32)
+    mcs = len(oy)
+    bnd = np.zeros(n_slabs + 1, dtype=np.int64)
+    lau = np.zeros((max(1, n_slabs) * 4 * mcs, 4), dtype=np.int64)
+    cop = np.zeros((n_slabs + 1, 3), dtype=np.int64)
+    ns, nl, nc = ctypes.c_uint32(), ctypes.c_uint32(), ctypes.c_uint32()
+    rc = load_library().kpz_overlap_plan(L, tile, mcs, n_slabs, oy.ctypes.data, bnd.ctypes.data, ctypes.addressof(ns),
+                                         lau.ctypes.data, ctypes.addressof(nl), cop.ctypes.data, ctypes.addressof(nc))
+    if rc != KPZ_OK:
+        raise KpzError(rc, "kpz_overlap_plan")
+    if ns.value == 0:
+        return None
+    return bnd[:ns.value + 1].copy(), lau[:nl.value].copy(), cop[:nc.value].copy()
 
 
 LAYOUT_NAMES = ("rows3_attempts_per_s", "rows3_warps_per_sm", "pitch66_attempts_per_s", "pitch66_warps_per_sm")

@@ -976,7 +976,111 @@ int32_t launch_pass_rows(kpz_ctx* c, uint32_t m, uint32_t slot, uint32_t cy, lon
     return c->T >= 32 ? kpz_launch_update_wide(c, P) : kpz_launch_update_narrow(c, P);
 }
 
+// The schedule of kpz_step_host_overlapped as plain host data (no CUDA): row boundaries of the blocks, the launches in
+// issue order (stage, pass, tile rows [a, b] of the frame of that pass's MCS, b may exceed NT - 1: wrapped range; the
+// colour of the pass then picks every second row), and the rows that may be copied back after each stage.
+// oy[m] = y offset of the global draw of the m-th MCS of the step.  False: the shape does not allow the overlap.
+struct OverlapLaunch { uint32_t stage, pass; long long a, b; };
+struct OverlapCopy { uint32_t stage; long long r0, r1; };
+struct OverlapPlan {
+    std::vector<long long> B;
+    std::vector<OverlapLaunch> launches;
+    std::vector<OverlapCopy> copies;
+};
+
+bool overlap_plan(long long L, long long T, long long mcs, long long n_slabs, const uint32_t* oy, OverlapPlan& pl) {
+    pl.B.clear();
+    pl.launches.clear();
+    pl.copies.clear();
+    if (mcs < 1 || n_slabs < 2 || T < 1 || L % (2 * T) != 0) return false;
+    const long long NT = L / T, P_ = 4 * mcs, step = T + 1;
+    // Block heights: compute is the bottleneck (the kernels of a step take about three times its copies), so only the
+    // FIRST copy-in and the LAST copy-out are exposed: the blocks ramp up geometrically (x2) from both ends and are
+    // large in the middle (few launches, little tail).  Every block must be taller than C_min.
+    const long long C_min = 2 * P_ * step + 4 * T;
+    bool eligible = false;
+    for (long long S_try = n_slabs; S_try >= 2 && !eligible; --S_try) {
+        std::vector<long long> w((size_t)S_try);
+        long long wsum = 0;
+        for (long long i = 0; i < S_try; ++i) {
+            const long long e = std::min(i, S_try - 1 - i);
+            w[(size_t)i] = 1ll << std::min<long long>(e, 20);
+            wsum += w[(size_t)i];
+        }
+        pl.B.assign(1, 0);
+        long long acc = 0;
+        bool ok = true;
+        for (long long i = 0; i < S_try; ++i) {
+            acc += w[(size_t)i];
+            const long long b = (i == S_try - 1) ? L : (L * acc / wsum) / (2 * T) * (2 * T);     // whole tile-row pairs
+            if (b - pl.B.back() < C_min) { ok = false; break; }
+            pl.B.push_back(b);
+        }
+        eligible = ok;
+    }
+    if (!eligible) { pl.B.clear(); return false; }
+    const std::vector<long long>& B = pl.B;
+    const long long S = (long long)B.size() - 1;
+    const long long g_last = (P_ - 1) * step;                               // g_{P-1}
+    long long out_next = g_last + T;                                        // first row not yet copied back
+    for (long long s = 0; s < S; ++s) {
+        for (long long p = 0; p < P_; ++p) {
+            const long long o = (long long)oy[p / 4];
+            const long long g = p * step;
+            const long long t_lo = ceil_div(g - o, T) < 0 ? 0 : ceil_div(g - o, T);
+            auto t_hi = [&](long long stage) { return floor_div((B[(size_t)stage + 1] - 1 - p * step) - T - o, T); };
+            long long a, b;
+            if (s < S - 1) {
+                a = s == 0 ? t_lo : std::max(t_lo, t_hi(s - 1) + 1);
+                b = t_hi(s);
+            } else {
+                a = std::max(t_lo, t_hi(S - 2) + 1);
+                b = NT - 1 + t_lo;                                          // wraps: tile rows 0 .. t_lo - 1 come last
+            }
+            if (b >= a) pl.launches.push_back({(uint32_t)s, (uint32_t)p, a, b});
+        }
+        if (s < S - 1) {
+            const long long hi = (B[(size_t)s + 1] - 1 - (P_ - 1) * step) - T;  // rows <= f_{s,P-1} - T are final
+            if (hi >= out_next) {
+                pl.copies.push_back({(uint32_t)s, out_next, hi});
+                out_next = hi + 1;
+            }
+        } else {
+            pl.copies.push_back({(uint32_t)s, out_next, L - 1});
+            pl.copies.push_back({(uint32_t)s, 0, g_last + T - 1});
+        }
+    }
+    return true;
+}
+
 }  // namespace
+
+int32_t kpz_overlap_plan(uint32_t L, uint32_t tile, uint64_t mcs, uint32_t n_slabs, const uint32_t* oy, int64_t* boundaries,
+                         uint32_t* n_stages, int64_t* launches, uint32_t* n_launches, int64_t* copies, uint32_t* n_copies) {
+    if (!oy || !boundaries || !n_stages || !launches || !n_launches || !copies || !n_copies) return KPZ_EINVAL;
+    if (L == 0 || tile == 0 || L % (2 * tile) != 0 || mcs == 0 || mcs > 0xFFFFFFFFull || n_slabs > 4096) return KPZ_EINVAL;
+    for (uint64_t m = 0; m < mcs; ++m)
+        if (oy[m] >= tile) return KPZ_EINVAL;
+    OverlapPlan pl;
+    *n_stages = *n_launches = *n_copies = 0;
+    if (!overlap_plan(L, tile, (long long)mcs, n_slabs, oy, pl)) return KPZ_OK;      // no overlap for this shape
+    *n_stages = (uint32_t)(pl.B.size() - 1);
+    for (size_t i = 0; i < pl.B.size(); ++i) boundaries[i] = pl.B[i];
+    *n_launches = (uint32_t)pl.launches.size();
+    for (size_t i = 0; i < pl.launches.size(); ++i) {
+        launches[4 * i + 0] = pl.launches[i].stage;
+        launches[4 * i + 1] = pl.launches[i].pass;
+        launches[4 * i + 2] = pl.launches[i].a;
+        launches[4 * i + 3] = pl.launches[i].b;
+    }
+    *n_copies = (uint32_t)pl.copies.size();
+    for (size_t i = 0; i < pl.copies.size(); ++i) {
+        copies[3 * i + 0] = pl.copies[i].stage;
+        copies[3 * i + 1] = pl.copies[i].r0;
+        copies[3 * i + 2] = pl.copies[i].r1;
+    }
+    return KPZ_OK;
+}
 
 int32_t kpz_step_host_overlapped(kpz_ctx* c, void* host_lattice, size_t bytes, int64_t* h00_inout, uint64_t mcs_start,
                                  uint64_t mcs, uint32_t n_slabs, int64_t* sum_h, int64_t* sum_h2, double* W2) {
@@ -985,40 +1089,27 @@ int32_t kpz_step_host_overlapped(kpz_ctx* c, void* host_lattice, size_t bytes, i
     DeviceGuard dg__(c->device);
     if ((rc = require_whole(c)) != KPZ_OK) return rc;
     if (!host_lattice || bytes < c->lattice_bytes || mcs_start + mcs > 0xFFFFFFFFull) return kpz_fail(c, KPZ_EINVAL, "bad argument");
-    const long long L = c->L, T = c->T, NT = L / T, P_ = 4 * (long long)mcs, step = T + 1;
-    ResidentPlan pl{};
-    // the overlap needs: one replica, the default schedule on the tiled kernel, and slabs much taller than the
-    // region the P passes eat away on both sides; otherwise the plain sequence (same result)
-    // Slab heights: compute is the bottleneck (the kernels of a step take about three times its copies), so only the
-    // FIRST copy-in and the LAST copy-out are exposed: the slabs ramp up geometrically (x2) from both ends and are
-    // large in the middle (few launches, little tail).  Every slab must be taller than C_min.
-    const long long C_min = 2 * P_ * step + 4 * T;
-    std::vector<long long> B;                                               // row boundaries B[0] = 0 .. B[S] = L
+    const long long L = c->L;
+    ResidentPlan rp{};
+    // the overlap needs: one replica, the default schedule on the tiled kernel, and blocks much taller than the
+    // region the passes of the step eat away on both sides (overlap_plan); otherwise the plain sequence (same result)
+    OverlapPlan plan;
+    std::vector<uint32_t> oy, cy;
     bool eligible = c->R == 1 && c->schedule == KPZ_SCHEDULE_COLOURS && c->sub_sweeps == 1 && !c->poisson && mcs >= 1 &&
-                    n_slabs >= 2 && choose_path(c, pl) == KPZ_PATH_TILED;
+                    n_slabs >= 2 && choose_path(c, rp) == KPZ_PATH_TILED;
     if (eligible) {
-        eligible = false;
-        for (long long S_try = n_slabs; S_try >= 2 && !eligible; --S_try) {
-            std::vector<long long> w((size_t)S_try);
-            long long wsum = 0;
-            for (long long i = 0; i < S_try; ++i) {
-                const long long e = std::min(i, S_try - 1 - i);
-                w[(size_t)i] = 1ll << std::min<long long>(e, 20);
-                wsum += w[(size_t)i];
-            }
-            B.assign(1, 0);
-            long long acc = 0;
-            bool ok = true;
-            for (long long i = 0; i < S_try; ++i) {
-                acc += w[(size_t)i];
-                const long long b = (i == S_try - 1) ? L : (L * acc / wsum) / (2 * T) * (2 * T);     // whole tile-row pairs
-                if (b - B.back() < C_min) { ok = false; break; }
-                B.push_back(b);
-            }
-            eligible = ok;
+        oy.resize((size_t)mcs);
+        cy.resize((size_t)(4 * mcs));
+        for (uint64_t m = 0; m < mcs; ++m) {
+            uint32_t ox, oyv, perm[4];
+            host_global_draw(c, (uint32_t)(mcs_start + m), 0u, 0u, &ox, &oyv, perm);
+            oy[(size_t)m] = oyv;
+            for (int slot = 0; slot < 4; ++slot) cy[(size_t)(4 * m) + slot] = perm[slot] >> 1;
         }
+        eligible = overlap_plan(L, c->T, (long long)mcs, n_slabs, oy.data(), plan);
     }
     if (!eligible) return kpz_step_host(c, host_lattice, bytes, h00_inout, mcs_start, mcs, sum_h, sum_h2, W2);
+    const std::vector<long long>& B = plan.B;
     const long long S = (long long)B.size() - 1;
     const size_t row_bytes = (size_t)L / 8, plane_bytes = (size_t)L * row_bytes;
     unsigned char* hb = static_cast<unsigned char*>(host_lattice);
@@ -1030,7 +1121,7 @@ int32_t kpz_step_host_overlapped(kpz_ctx* c, void* host_lattice, size_t bytes, i
     cudaEvent_t* ev_cmp = c->events.data() + S;
     c->mcs = mcs_start;
     c->attempts_base = mcs_start * (uint64_t)c->L * c->L;
-    // all slabs are queued on the copy-in stream at once: they arrive in order
+    // all blocks are queued on the copy-in stream at once: they arrive in order
     for (long long s = 0; s < S; ++s) {
         for (int pln = 0; pln < 2; ++pln) {
             const size_t off = pln * plane_bytes + (size_t)B[(size_t)s] * row_bytes;
@@ -1039,45 +1130,22 @@ int32_t kpz_step_host_overlapped(kpz_ctx* c, void* host_lattice, size_t bytes, i
         }
         KPZ_CUDA(c, cudaEventRecord(ev_in[s], c->s_in));
     }
-    auto copy_out_rows = [&](long long r0, long long r1) -> int32_t {      // rows [r0, r1] of both planes
-        if (r1 < r0) return KPZ_OK;
-        for (int pln = 0; pln < 2; ++pln) {
-            const size_t off = pln * plane_bytes + (size_t)r0 * row_bytes;
-            KPZ_CUDA(c, cudaMemcpyAsync(hb + off, db + off, (size_t)(r1 - r0 + 1) * row_bytes, cudaMemcpyDeviceToHost, c->s_out));
-        }
-        return KPZ_OK;
-    };
-    const long long g_last = (P_ - 1) * step;                               // g_{P-1}
-    long long out_next = g_last + T;                                        // first row not yet copied back
+    size_t li = 0, ci = 0;
     for (long long s = 0; s < S; ++s) {
         KPZ_CUDA(c, cudaStreamWaitEvent(c->stream, ev_in[s], 0));
-        for (long long p = 0; p < P_; ++p) {
-            const uint32_t m = (uint32_t)(mcs_start + (uint64_t)(p / 4)), slot = (uint32_t)(p % 4);
-            uint32_t ox, oy, perm[4];
-            host_global_draw(c, m, 0u, 0u, &ox, &oy, perm);
-            const uint32_t cy = perm[slot] >> 1;
-            const long long g = p * step;
-            const long long t_lo = ceil_div(g - (long long)oy, T) < 0 ? 0 : ceil_div(g - (long long)oy, T);
-            auto t_hi = [&](long long stage) { return floor_div((B[(size_t)stage + 1] - 1 - p * step) - T - (long long)oy, T); };
-            long long a, b;
-            if (s < S - 1) {
-                a = s == 0 ? t_lo : std::max(t_lo, t_hi(s - 1) + 1);
-                b = t_hi(s);
-            } else {
-                a = std::max(t_lo, t_hi(S - 2) + 1);
-                b = NT - 1 + t_lo;                                          // wraps: tile rows 0 .. t_lo - 1 come last
-            }
-            if ((rc = launch_pass_rows(c, m, slot, cy, a, b)) != KPZ_OK) return rc;
+        for (; li < plan.launches.size() && plan.launches[li].stage == (uint32_t)s; ++li) {
+            const OverlapLaunch& ln = plan.launches[li];
+            const uint32_t m = (uint32_t)(mcs_start + (uint64_t)(ln.pass / 4)), slot = ln.pass % 4;
+            if ((rc = launch_pass_rows(c, m, slot, cy[ln.pass], ln.a, ln.b)) != KPZ_OK) return rc;
         }
         KPZ_CUDA(c, cudaEventRecord(ev_cmp[s], c->stream));
         KPZ_CUDA(c, cudaStreamWaitEvent(c->s_out, ev_cmp[s], 0));
-        if (s < S - 1) {
-            const long long hi = (B[(size_t)s + 1] - 1 - (P_ - 1) * step) - T;  // rows <= f_{s,P-1} - T are final
-            if ((rc = copy_out_rows(out_next, hi)) != KPZ_OK) return rc;
-            if (hi >= out_next) out_next = hi + 1;
-        } else {
-            if ((rc = copy_out_rows(out_next, L - 1)) != KPZ_OK) return rc;
-            if ((rc = copy_out_rows(0, g_last + T - 1)) != KPZ_OK) return rc;
+        for (; ci < plan.copies.size() && plan.copies[ci].stage == (uint32_t)s; ++ci) {
+            const OverlapCopy& cp = plan.copies[ci];                         // rows [r0, r1] of both planes
+            for (int pln = 0; pln < 2; ++pln) {
+                const size_t off = pln * plane_bytes + (size_t)cp.r0 * row_bytes;
+                KPZ_CUDA(c, cudaMemcpyAsync(hb + off, db + off, (size_t)(cp.r1 - cp.r0 + 1) * row_bytes, cudaMemcpyDeviceToHost, c->s_out));
+            }
         }
     }
     c->mcs = mcs_start + mcs;
