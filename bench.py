@@ -552,7 +552,7 @@ def main():
                                                         "runs the paper's own 8 x 8 cells)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--pipeline", action="store_true", help="also time kpz_pipeline_host for configs other than 3")
-    ap.add_argument("--e2e-slabs", type=int, default=8, help="row slabs of kpz_step_host_overlapped in the e2e leg")
+    ap.add_argument("--e2e-slabs", type=int, default=5, help="row slabs of kpz_step_host_overlapped in the e2e leg")
     ap.add_argument("--peaks", action="store_true", help="print the pipe micro-benchmarks (kpz_measure_peaks) and exit")
     ap.add_argument("--layouts", action="store_true", help="print the tile-layout experiment (kpz_measure_layouts) and exit")
     ap.add_argument("--slabs", action="store_true", help="ONE lattice of the config split into slabs of rows over the N ranks "

@@ -214,7 +214,9 @@ int32_t kpz_step_host_overlapped(kpz_ctx* ctx, void* host_lattice, size_t bytes,
 
 /* The schedule kpz_step_host_overlapped follows, as plain HOST data (no device, no handle: host logic, checked exhaustively
  * in tests/test_overlap_plan.py).  Inputs: lattice edge L, tile edge (L a multiple of 2 * tile), mcs >= 1 MCS per step,
- * the requested number of blocks n_slabs, and oy[m] < tile, the y offset of the global draw of the m-th MCS of the step
+ * the requested number of blocks n_slabs, wave_tiles = the tiles the GPU holds at a time (SMs x resident tiles per SM; the
+ * blocks away from the middle are then whole numbers of such waves, so that their launches end on a full wave; 0: blocks in
+ * proportion 1 : 2 : 4 .. : 4 : 2 : 1), and oy[m] < tile, the y offset of the global draw of the m-th MCS of the step
  * (kpz_global_draw).  Outputs, all HOST arrays owned by the caller:
  *   boundaries[*n_stages + 1] : block s holds lattice rows boundaries[s] .. boundaries[s + 1] - 1 (capacity n_slabs + 1)
  *   launches[*n_launches][4]  : in issue order: stage, pass p = 4 m + colour slot, first and last tile row of the
@@ -224,8 +226,9 @@ int32_t kpz_step_host_overlapped(kpz_ctx* ctx, void* host_lattice, size_t bytes,
  * *n_stages = 0 (and KPZ_OK) when the shape does not allow the overlap (blocks would be shorter than
  * 8 mcs (tile + 1) + 4 tile rows even for two blocks): kpz_step_host_overlapped then is kpz_step_host.
  * KPZ_EINVAL: NULL pointer, L not a multiple of 2 * tile, mcs = 0, an offset >= tile, n_slabs > 4096. */
-int32_t kpz_overlap_plan(uint32_t L, uint32_t tile, uint64_t mcs, uint32_t n_slabs, const uint32_t* oy, int64_t* boundaries,
-                         uint32_t* n_stages, int64_t* launches, uint32_t* n_launches, int64_t* copies, uint32_t* n_copies);
+int32_t kpz_overlap_plan(uint32_t L, uint32_t tile, uint64_t mcs, uint32_t n_slabs, uint32_t wave_tiles, const uint32_t* oy,
+                         int64_t* boundaries, uint32_t* n_stages, int64_t* launches, uint32_t* n_launches, int64_t* copies,
+                         uint32_t* n_copies);
 
 /* Pipelined end-to-end steps with HOST buffers: n_lanes independent lattices
  * (same L, p, q, tile, seed as the handle; they differ in state and MCS clock), each a HOST buffer of `bytes` >=

@@ -76,7 +76,7 @@ def load_library() -> ctypes.CDLL:
         "kpz_philox_selftest": [vp, vp, vp, u32],
         "kpz_measure_peaks": [vp, u32],
         "kpz_measure_layouts": [vp, u32],
-        "kpz_overlap_plan": [u32, u32, u64, u32, vp, vp, vp, vp, vp, vp, vp],
+        "kpz_overlap_plan": [u32, u32, u64, u32, u32, vp, vp, vp, vp, vp, vp, vp],
         "kpz_slab_workspace_bytes": [u32, u32, u32, vp, vp],
         "kpz_create_slab": [vp, u32, dbl, dbl, u32, u64, u32, u32],
         "kpz_slab_info": [vp, vp, vp, vp, vp, vp],
@@ -120,7 +120,7 @@ def measure_peaks():
     return dict(zip(PEAK_NAMES, out.tolist()))
 
 
-def overlap_plan(L, tile, oy, n_slabs):
+def overlap_plan(L, tile, oy, n_slabs, wave_tiles=0):
     """kpz_overlap_plan (host only): the schedule of kpz_step_host_overlapped for a step of len(oy) MCS with y offsets oy.
     -> (boundaries, launches[n][4] = stage, pass, first, last tile row, copies[n][3] = stage, first, last row), or None
     when the shape does not allow the overlap."""
@@ -130,7 +130,7 @@ def overlap_plan(L, tile, oy, n_slabs):
     lau = np.zeros((max(1, n_slabs) * 4 * mcs, 4), dtype=np.int64)
     cop = np.zeros((n_slabs + 1, 3), dtype=np.int64)
     ns, nl, nc = ctypes.c_uint32(), ctypes.c_uint32(), ctypes.c_uint32()
-    rc = load_library().kpz_overlap_plan(L, tile, mcs, n_slabs, oy.ctypes.data, bnd.ctypes.data, ctypes.addressof(ns),
+    rc = load_library().kpz_overlap_plan(L, tile, mcs, n_slabs, wave_tiles, oy.ctypes.data, bnd.ctypes.data, ctypes.addressof(ns),
                                          lau.ctypes.data, ctypes.addressof(nl), cop.ctypes.data, ctypes.addressof(nc))
     if rc != KPZ_OK:
         raise KpzError(rc, "kpz_overlap_plan")

@@ -988,7 +988,8 @@ struct OverlapPlan {
     std::vector<OverlapCopy> copies;
 };
 
-bool overlap_plan(long long L, long long T, long long mcs, long long n_slabs, const uint32_t* oy, OverlapPlan& pl) {
+bool overlap_plan(long long L, long long T, long long mcs, long long n_slabs, long long wave_tiles, const uint32_t* oy,
+                  OverlapPlan& pl) {
     pl.B.clear();
     pl.launches.clear();
     pl.copies.clear();
@@ -999,6 +1000,32 @@ bool overlap_plan(long long L, long long T, long long mcs, long long n_slabs, co
     // large in the middle (few launches, little tail).  Every block must be taller than C_min.
     const long long C_min = 2 * P_ * step + 4 * T;
     bool eligible = false;
+    // (a) whole waves: a launch of a middle stage covers (block height / 2T) tile rows of its colour, L / 2T tiles each;
+    // the GPU holds wave_tiles tiles at a time, so a block of k waves minus a bit wastes nothing in the last wave of its
+    // 4 mcs launches.  Blocks of kmin, 2 kmin, 4 kmin .. waves from both ends, the middle block takes the rest.
+    const double q = wave_tiles > 0 ? (double)wave_tiles / (double)(L / (2 * T)) : 0.0;      // colour rows per wave
+    if (q >= 1.0) {
+        auto rows_for = [&](long long k) { return (long long)std::floor((double)k * q) * 2 * T; };
+        long long kmin = 1;
+        while (rows_for(kmin) < C_min) ++kmin;
+        for (long long S_try = n_slabs; S_try >= 3 && !eligible; --S_try) {
+            const long long mid = S_try / 2;
+            std::vector<long long> h((size_t)S_try, 0);
+            long long sum = 0;
+            for (long long i = 0; i < S_try; ++i) {
+                if (i == mid) continue;
+                const long long e = std::min(i, S_try - 1 - i);
+                h[(size_t)i] = rows_for(kmin << std::min<long long>(e, 20));
+                sum += h[(size_t)i];
+            }
+            h[(size_t)mid] = L - sum;
+            if (h[(size_t)mid] < C_min) continue;
+            pl.B.assign(1, 0);
+            for (long long i = 0; i < S_try; ++i) pl.B.push_back(pl.B.back() + h[(size_t)i]);
+            eligible = true;
+        }
+    }
+    // (b) otherwise in proportion 1 : 2 : 4 .. : 4 : 2 : 1
     for (long long S_try = n_slabs; S_try >= 2 && !eligible; --S_try) {
         std::vector<long long> w((size_t)S_try);
         long long wsum = 0;
@@ -1055,15 +1082,16 @@ bool overlap_plan(long long L, long long T, long long mcs, long long n_slabs, co
 
 }  // namespace
 
-int32_t kpz_overlap_plan(uint32_t L, uint32_t tile, uint64_t mcs, uint32_t n_slabs, const uint32_t* oy, int64_t* boundaries,
-                         uint32_t* n_stages, int64_t* launches, uint32_t* n_launches, int64_t* copies, uint32_t* n_copies) {
+int32_t kpz_overlap_plan(uint32_t L, uint32_t tile, uint64_t mcs, uint32_t n_slabs, uint32_t wave_tiles, const uint32_t* oy,
+                         int64_t* boundaries, uint32_t* n_stages, int64_t* launches, uint32_t* n_launches, int64_t* copies,
+                         uint32_t* n_copies) {
     if (!oy || !boundaries || !n_stages || !launches || !n_launches || !copies || !n_copies) return KPZ_EINVAL;
     if (L == 0 || tile == 0 || L % (2 * tile) != 0 || mcs == 0 || mcs > 0xFFFFFFFFull || n_slabs > 4096) return KPZ_EINVAL;
     for (uint64_t m = 0; m < mcs; ++m)
         if (oy[m] >= tile) return KPZ_EINVAL;
     OverlapPlan pl;
     *n_stages = *n_launches = *n_copies = 0;
-    if (!overlap_plan(L, tile, (long long)mcs, n_slabs, oy, pl)) return KPZ_OK;      // no overlap for this shape
+    if (!overlap_plan(L, tile, (long long)mcs, n_slabs, wave_tiles, oy, pl)) return KPZ_OK;      // no overlap for this shape
     *n_stages = (uint32_t)(pl.B.size() - 1);
     for (size_t i = 0; i < pl.B.size(); ++i) boundaries[i] = pl.B[i];
     *n_launches = (uint32_t)pl.launches.size();
@@ -1106,7 +1134,12 @@ int32_t kpz_step_host_overlapped(kpz_ctx* c, void* host_lattice, size_t bytes, i
             oy[(size_t)m] = oyv;
             for (int slot = 0; slot < 4; ++slot) cy[(size_t)(4 * m) + slot] = perm[slot] >> 1;
         }
-        eligible = overlap_plan(L, c->T, (long long)mcs, n_slabs, oy.data(), plan);
+        // tiles one wave of the update kernel holds (its CTA shapes: kpz_launch_update_wide.cu): blocks of whole waves
+        int sms = 0;
+        KPZ_CUDA(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device));
+        const long long per_sm = c->T == 64 ? 288 : (c->T == 32 ? 512 : 0);
+        const long long wave_tiles = (long long)sms * per_sm;
+        eligible = overlap_plan(L, c->T, (long long)mcs, n_slabs, wave_tiles, oy.data(), plan);
     }
     if (!eligible) return kpz_step_host(c, host_lattice, bytes, h00_inout, mcs_start, mcs, sum_h, sum_h2, W2);
     const std::vector<long long>& B = plan.B;

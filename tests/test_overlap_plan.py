@@ -101,7 +101,9 @@ def test_overlap_plan_is_a_valid_schedule(pkg, L, T, mcs, n_slabs):
         if trial == 1:
             oy[:] = T - 4 if T >= 4 else T - 1
         cy = np.concatenate([(rng.permutation(4) >> 1) for _ in range(mcs)]).astype(np.uint32)
-        plan = pkg.overlap_plan(L, T, oy, n_slabs)
+        # blocks in proportion 1 : 2 : 4 .. (wave_tiles = 0) or as whole waves of a GPU that holds wave_tiles tiles
+        wave_tiles = (0, 148 * 288, 148 * 512, 1000, 37 * L // (2 * T))[(trial + mcs) % 5]
+        plan = pkg.overlap_plan(L, T, oy, n_slabs, wave_tiles)
         assert plan is not None
         S = _replay(L, T, oy, cy, plan)
         assert 2 <= S <= n_slabs
@@ -130,3 +132,21 @@ def test_overlap_plan_blocks_ramp_up_from_both_ends(pkg):
     mid = len(h) // 2
     assert np.all(np.diff(h[:mid + 1]) >= 0) and np.all(np.diff(h[mid:]) <= 0)
     assert h[0] < h[mid] / 2 and h[-1] < h[mid] / 2
+    # whole waves: with 148 SMs x 288 tiles a wave is 41.625 tile rows of one colour at L = 2^17, T = 64; every block but
+    # the middle one is the largest whole number of tile-row pairs below 2, 4, 8 .. waves
+    wave = 148 * 288
+    bnd, launches, _ = pkg.overlap_plan(1 << 17, 64, np.zeros(10, dtype=np.uint32), 8, wave)
+    h = np.diff(bnd)
+    mid = len(h) // 2
+    per_row = (1 << 17) // 128                     # tiles of one colour in a tile row
+    for i, rows in enumerate(h):
+        if i == mid:
+            continue
+        k = 2 << min(i, len(h) - 1 - i)
+        assert rows == (k * wave // per_row) * 128
+    # a middle stage launches (block height / 128) colour rows per pass: just under a whole number of waves
+    st = launches[launches[:, 0] == 1]
+    assert len(st) == 40
+    for _, _, a, b in st:
+        colour_rows = (b - a + 1 + 1) // 2
+        assert colour_rows * per_row <= 4 * wave
