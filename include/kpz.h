@@ -206,7 +206,8 @@ int32_t kpz_step_host(kpz_ctx* ctx, void* host_lattice, size_t bytes, int64_t* h
  * copied back while later blocks still compute, and the last stage completes the rest in pass order.  Same kernels,
  * same results as kpz_step_host, bit for bit.  host_lattice should be pinned memory (pageable memory makes the copies
  * synchronous: still correct, no overlap).  The n_slabs blocks ramp up in height (x2) from both ends of the lattice, so that
- * only a short first copy-in and a short last copy-out are exposed.  Needs n_replicas = 1, the default schedule on the tiled
+ * only a short first copy-in and a short last copy-out are exposed; for tile = 64 and 32 they are whole numbers of waves of
+ * the tiles the GPU holds at a time (kpz_overlap_plan has the schedule as data).  Needs n_replicas = 1, the default schedule on the tiled
  * kernel, n_slabs >= 2 and every block taller than 8 mcs (tile + 1) + 4 tile rows (n_slabs is reduced until that holds);
  * otherwise it IS kpz_step_host.  Synchronises before returning. */
 int32_t kpz_step_host_overlapped(kpz_ctx* ctx, void* host_lattice, size_t bytes, int64_t* h00_inout, uint64_t mcs_start,
