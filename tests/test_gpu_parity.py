@@ -348,6 +348,35 @@ def test_config4_replicas_2000_mcs_in_one_launch(pkg):
     _compare_full(k, os_[R - 1], replica=R - 1)
 
 
+@pytest.mark.parametrize("L,T,R,n", [(128, 8, 64, 300), (256, 8, 12, 120), (128, 4, 16, 150), (512, 8, 3, 40)])
+def test_replica_batch_small_tiles_resident_and_tiled(pkg, L, T, R, n):
+    """Config 4 with the paper's own 8 x 8 cells (the configuration of profiles/r02_config4_fss_t8.md and of the 400 / 540
+    Gupd/s figures) and with 4 x 4: n MCS in ONE launch of the lattice-resident kernel, then 3 more, every replica against
+    the oracle; the tiled kernel on the same handle parameters must land on the same states."""
+    seed = 4
+    k = pkg.KPZ(L, 1.0, 0.0, T, seed, n_replicas=R)
+    k.init_flat()
+    l0 = k.launch_count()
+    k.run(n)
+    assert k.launch_count() - l0 == 1            # lattice-resident: one launch for the whole call
+    k.run(3)
+    os_ = [Oracle(L, 1.0, 0.0, T, seed, replica=r, threads=NTHREADS) for r in range(R)]
+    for o in os_:
+        o.init_flat(); o.run(n + 3)
+    _compare_scalars(k, os_)
+    for r in range(R):
+        assert k.state_hash(r) == os_[r].state_hash()
+        assert k.counters(r) == os_[r].counters()
+    _compare_full(k, os_[R - 1], replica=R - 1)
+    t = pkg.KPZ(L, 1.0, 0.0, T, seed, n_replicas=R)
+    t.set_path("tiled")
+    t.init_flat()
+    t.run(n + 3)
+    for r in range(R):
+        assert t.state_hash(r) == os_[r].state_hash()
+    k.close(); t.close()
+
+
 def test_replica_batch_1024_general_pq(pkg):
     L, T, seed, R, n = 128, 16, 4, 1024, 3
     k = pkg.KPZ(L, 0.75, 0.25, T, seed, n_replicas=R)
